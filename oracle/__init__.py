@@ -1,0 +1,168 @@
+"""ctypes loader for the oracle (oracle/oracle.cpp).  TEST INFRASTRUCTURE, NOT PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this.  It imports nothing from paper_1011_2188_b200 (the CUDA path) and vice versa.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+FLAG_RANDOM_AZIMUTH = 1
+
+
+class TrackDBStruct(ctypes.Structure):
+    _fields_ = [("dx", ctypes.c_void_p), ("dy", ctypes.c_void_p), ("dz", ctypes.c_void_p),
+                ("dE", ctypes.c_void_p), ("E", ctypes.c_void_p), ("n_steps", ctypes.c_uint64),
+                ("track_off", ctypes.c_void_p), ("n_tracks", ctypes.c_uint32),
+                ("bin_first", ctypes.c_void_p), ("n_bins", ctypes.c_uint32),
+                ("e_min", ctypes.c_float), ("e_bin", ctypes.c_float)]
+
+
+class StatsStruct(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_uint64) for n in ("protons", "proton_steps", "deposits", "missed", "escaped",
+                                               "stopped", "grid_sum", "q_replayed", "q_escaped")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -ffp-contract=off (the arithmetic contract)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        subprocess.check_call(["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math",
+                               "-shared", "-fPIC", "-o", tmp, _SRC])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        L.oracle_signed_unit.restype = ctypes.c_float
+        L.oracle_signed_unit.argtypes = [ctypes.c_uint32]
+        L.oracle_ln.restype = ctypes.c_double
+        L.oracle_ln.argtypes = [ctypes.c_double]
+        L.oracle_energy_bin.restype = ctypes.c_int
+        L.oracle_energy_bin.argtypes = [ctypes.c_float] * 3
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return ctypes.c_void_p(a.ctypes.data)
+
+
+def philox(ctr, key):
+    c = np.asarray(ctr, dtype=np.uint32); k = np.asarray(key, dtype=np.uint32); o = np.zeros(4, dtype=np.uint32)
+    lib().oracle_philox4x32_10(_p(c), _p(k), _p(o))
+    return o
+
+
+def material_lut(table):
+    t = np.ascontiguousarray(table)
+    rho, w, f = (np.zeros(4096, dtype=np.float32) for _ in range(3))
+    lib().oracle_material_lut(_p(t), ctypes.c_int(len(t)), _p(rho), _p(w), _p(f))
+    return rho, w, f
+
+
+def _db_struct(db):
+    arrs = [np.ascontiguousarray(a, dtype=np.float32) for a in (db.dx, db.dy, db.dz, db.dE, db.E)]
+    off = np.ascontiguousarray(db.track_off, dtype=np.uint64)
+    bf = np.ascontiguousarray(db.bin_first, dtype=np.uint32)
+    s = TrackDBStruct(*[a.ctypes.data for a in arrs], arrs[0].shape[0], off.ctypes.data, off.shape[0] - 1,
+                      bf.ctypes.data, bf.shape[0] - 1, db.e_min, db.e_bin)
+    return s, (arrs, off, bf)
+
+
+def _common_args(phantom, table, db, beamlets):
+    hu = np.ascontiguousarray(phantom.hu, dtype=np.int16)
+    nx, ny, nz = phantom.dims
+    t = np.ascontiguousarray(table)
+    bl = np.ascontiguousarray(beamlets)
+    dbs, keep = _db_struct(db)
+    args = [_p(hu), ctypes.c_int(nx), ctypes.c_int(ny), ctypes.c_int(nz)] + \
+           [ctypes.c_float(s) for s in phantom.spacing] + \
+           [_p(t), ctypes.c_int(len(t)), ctypes.byref(dbs), _p(bl), ctypes.c_uint32(len(bl))]
+    return args, (hu, t, bl, dbs, keep)
+
+
+def _range_args(first, n, stride, seed, flags):
+    return [ctypes.c_uint64(first), ctypes.c_uint64(n), ctypes.c_uint64(stride), ctypes.c_uint64(seed),
+            ctypes.c_uint32(flags)]
+
+
+def run(phantom, table, db, beamlets, seed, first=0, n=None, stride=1, flags=FLAG_RANDOM_AZIMUTH,
+        grid=None, f64=False, end_state=False):
+    """Whole path, single thread.  Returns (grid u64 [nz,ny,nx], stats dict[, end_state])."""
+    if n is None:
+        n = int(beamlets["n_protons"].sum()) - first
+    if grid is None:
+        grid = np.zeros(phantom.hu.shape, dtype=np.uint64)
+    st = StatsStruct()
+    a, keep = _common_args(phantom, table, db, beamlets)
+    a += _range_args(first, n, stride, seed, flags) + [_p(grid), ctypes.byref(st)]
+    es = None
+    if f64:
+        es = np.zeros((n, 6), dtype=np.float64) if end_state else None
+        a.append(_p(es) if es is not None else None)
+        rc = lib().oracle_run_f64(*a)
+    else:
+        rc = lib().oracle_run(*a)
+    if rc != 0:
+        raise RuntimeError("oracle_run failed rc=%d" % rc)
+    d = st.as_dict()
+    d["grid_sum"] = int(grid.sum(dtype=np.uint64))
+    return (grid, d, es) if (f64 and end_state) else (grid, d)
+
+
+def run_trace(phantom, table, db, beamlets, seed, first=0, n=1, stride=1, flags=FLAG_RANDOM_AZIMUTH, cap=1 << 20):
+    """f32 run recording every deposit: returns grid, stats, (voxel, share, step), end_state[n,6]."""
+    grid = np.zeros(phantom.hu.shape, dtype=np.uint64)
+    st = StatsStruct()
+    vox = np.zeros(cap, dtype=np.uint64); share = np.zeros(cap, dtype=np.uint64); step = np.zeros(cap, dtype=np.uint32)
+    ntr = ctypes.c_uint64(0)
+    es = np.zeros((n, 6), dtype=np.float32)
+    a, keep = _common_args(phantom, table, db, beamlets)
+    a += _range_args(first, n, stride, seed, flags) + [_p(grid), ctypes.byref(st), _p(vox), _p(share), _p(step),
+                                                        ctypes.c_uint64(cap), ctypes.byref(ntr), _p(es)]
+    rc = lib().oracle_run_trace(*a)
+    if rc != 0:
+        raise RuntimeError("oracle_run_trace failed rc=%d" % rc)
+    k = int(ntr.value)
+    d = st.as_dict(); d["grid_sum"] = int(grid.sum(dtype=np.uint64))
+    return grid, d, (vox[:k], share[:k], step[:k]), es
+
+
+def sample(phantom, table, db, beamlets, seed, first=0, n=1, stride=1, flags=FLAG_RANDOM_AZIMUTH):
+    """R2-R6 only: per-proton start state."""
+    out = dict(beamlet=np.zeros(n, np.uint32), track=np.zeros(n, np.uint32), k0=np.zeros(n, np.uint64),
+               p=np.zeros((n, 3), np.float32), R=np.zeros((n, 3, 3), np.float32), iv=np.zeros((n, 3), np.int32),
+               missed=np.zeros(n, np.int32), csg=np.zeros((n, 4), np.float32))
+    a, keep = _common_args(phantom, table, db, beamlets)
+    a += _range_args(first, n, stride, seed, flags)
+    a += [_p(out[k]) for k in ("beamlet", "track", "k0", "p", "R", "iv", "missed", "csg")]
+    rc = lib().oracle_sample(*a)
+    if rc != 0:
+        raise RuntimeError("oracle_sample failed rc=%d" % rc)
+    return out
+
+
+def to_gy(grid, phantom, table):
+    hu = np.ascontiguousarray(phantom.hu, dtype=np.int16)
+    g = np.ascontiguousarray(grid, dtype=np.uint64)
+    t = np.ascontiguousarray(table)
+    dose = np.zeros(hu.shape, dtype=np.float32)
+    lib().oracle_to_gy(_p(g), _p(hu), ctypes.c_uint64(g.size), *[ctypes.c_float(s) for s in phantom.spacing],
+                       _p(t), ctypes.c_int(len(t)), _p(dose))
+    return dose
