@@ -1,0 +1,160 @@
+/*
+ * fdc.h -- C-ABI boundary of the B200-native track-repeating proton dose engine.
+ *
+ * The hot path of Yepes, Mirkovic & Taddei, "A GPU implementation of a track-repeating algorithm
+ * for proton radiotherapy dose calculations", as named by BASELINE.json:north_star:
+ *   fdc_create(CT HU grid, voxel spacing, HU -> density / stopping-power / scattering-power table)
+ *   fdc_load_tracks(SoA track database binned by incident energy)
+ *   fdc_run(beam fields, proton count, seed) -> dose grid
+ * What each call computes is defined rule by rule in DESIGN.md §3 (R1-R9); citations below are
+ * PAPER.md line numbers.  Every stage runs in CUDA kernels compiled for sm_100a; there is no CPU
+ * fallback (FDC_EARCH on any other device).
+ *
+ * Conventions: mm, MeV, g/cm^3.  The grid occupies [0,nx*sx] x [0,ny*sy] x [0,nz*sz]; voxel
+ * (ix,iy,iz) has linear index ix + nx*(iy + ny*iz) (x fastest) in every array crossing this ABI.
+ * All calls are asynchronous on the context's stream except where they return host data, in which
+ * case they synchronise that stream before returning.  Functions return 0 or a negative FDC_E*
+ * code; they never abort or throw, and leave no partial state behind on failure.
+ */
+#ifndef FDC_H
+#define FDC_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fdc_ctx fdc_ctx;                 /* opaque; one per device */
+
+/* Knot of the piecewise-linear HU -> material table ("scaling parameters of the step
+ * length and scattering angle for all the materials"; L98 density from HU).  mass_spr / mass_scpr:
+ * mass stopping-power / mass scattering-power ratio to water (R1). */
+typedef struct { float hu, density_g_cc, mass_spr, mass_scpr; } fdc_knot;
+
+/* Database of pre-computed water tracks (per step "the direction, length and energy
+ * loss is stored"), SoA, binned by incident energy.  Step k: displacement (dx,dy,dz) mm, energy
+ * loss dE MeV, E[k] = kinetic energy at the start of the step.  Track j owns steps
+ * [track_off[j], track_off[j+1]); bin b owns tracks [bin_first[b], bin_first[b+1]) and has nominal
+ * energy e_min_mev + b*e_bin_mev.  Requirements (else FDC_EINVAL): offsets non-decreasing and
+ * consistent with n_steps / n_tracks; within a track E non-increasing; 0 <= dE < 256; step length
+ * either 0 or within [1e-12, 1e6] mm; all values finite. */
+typedef struct {
+    const float *dx, *dy, *dz, *dE, *E;         /* n_steps each */
+    uint64_t n_steps;
+    const uint64_t *track_off;                  /* n_tracks + 1 */
+    uint32_t n_tracks;
+    const uint32_t *bin_first;                  /* n_bins + 1 */
+    uint32_t n_bins;
+    float e_min_mev, e_bin_mev;
+} fdc_trackdb;
+
+/* One (field, energy layer, spot) of a beam plan -- the paper's phase-space generator with fixed
+ * energy and direction and a transverse position spread.  (e1, e2, dir) must be
+ * orthonormal within 1e-5 with e1 x e2 = dir.  Protons start at
+ * origin + (spot_u + N(0,sigma)) e1 + (spot_v + N(0,sigma)) e2 and travel along dir. */
+typedef struct {
+    float origin[3], e1[3], e2[3], dir[3];
+    float energy_mev, spot_u_mm, spot_v_mm, sigma_mm;
+    uint64_t n_protons;
+} fdc_beamlet;
+
+typedef struct {
+    uint64_t protons;        /* protons executed */
+    uint64_t proton_steps;   /* database steps begun */
+    uint64_t deposits;       /* non-zero shares added to the grid (atomic operations) */
+    uint64_t missed;         /* never entered the grid */
+    uint64_t escaped;        /* left the grid before the track ended */
+    uint64_t stopped;        /* track ended inside the grid */
+    uint64_t grid_sum;       /* sum of the fixed-point grid (computed by fdc_get_stats) */
+    uint64_t q_replayed;     /* sum of Q over all steps from each proton's start step on */
+    uint64_t q_escaped;      /* part of q_replayed not tallied because the proton escaped;
+                                grid_sum + q_escaped == q_replayed exactly (R8) */
+} fdc_stats;
+
+enum {
+    FDC_OK        =  0,
+    FDC_EINVAL    = -1,   /* null pointer, bad size / spacing / table / frame / proton range, stride 0 */
+    FDC_ENOTRACKS = -2,   /* fdc_run before fdc_load_tracks */
+    FDC_ERANGE    = -3,   /* beamlet energy above the top bin, or its bin is empty */
+    FDC_ENOMEM    = -4,
+    FDC_ECUDA     = -5,   /* CUDA error; text via fdc_last_error */
+    FDC_EARCH     = -6    /* device is not compute capability 10.x (no fallback by design) */
+};
+
+enum {
+    FDC_RANDOM_AZIMUTH = 1u,   /* rotate each re-used track by a random azimuth about the beam (R5) */
+    FDC_DOSE_TO_HOST   = 2u,   /* dose_gy is a host pointer (else device) */
+    FDC_NO_SORT        = 4u,   /* debug: do not group protons by track (same result, slower) */
+    FDC_NO_AGGREGATE   = 8u    /* debug: one atomic per share, no warp aggregation (same result) */
+};
+
+/*
+ * Create a context on `device` using `cuda_stream` (a cudaStream_t; NULL = default stream).
+ * hu: nx*ny*nz int16 Hounsfield units, x fastest ("three dimensional array with a
+ * material index for each voxel"); values are clamped to [-1024, 3071].  If hu_is_device_ptr the
+ * array is BORROWED for the life of the context (the caller keeps it alive and unchanged); a host
+ * array is copied before return.  table: n_knots >= 1 knots, strictly increasing in hu, all of
+ * density, mass_spr, mass_scpr > 0 (host pointer, copied).  Builds the material LUT (R1) and a
+ * zeroed u64 energy grid (quantum 2^-24 MeV).
+ */
+int fdc_create(fdc_ctx **out, int device, void *cuda_stream,
+               const int16_t *hu, int nx, int ny, int nz, float sx, float sy, float sz,
+               const fdc_knot *table, int n_knots, int hu_is_device_ptr);
+
+/* Load (replace) the track database.  The five step arrays are host or device pointers per
+ * arrays_are_device_ptrs; track_off and bin_first are always host pointers.  Nothing is borrowed:
+ * the library derives its own device-resident step store (unit direction, length, fixed-point
+ * energy, suffix sums) before returning, so the caller may free its arrays afterwards. */
+int fdc_load_tracks(fdc_ctx *ctx, const fdc_trackdb *db, int arrays_are_device_ptrs);
+
+/*
+ * Transport protons and ADD their energy deposits to the context's grid.
+ * b[0..n_beamlets) (host) defines the global proton index space [0, sum n_protons); the call
+ * executes indices first_proton + m*proton_stride for m in [0, n_protons), all of which must lie
+ * in that space.  Proton i draws the same random numbers whatever the call that executes it
+ * (Philox4x32-10 keyed by seed, counter i; R3), so run(0..N) == run(0..a) + run(a..N) bit for bit.
+ * If dose_gy is not NULL it receives nx*ny*nz floats: the grid as it stands after this call
+ * converted to Gy (R9) -- device memory, or host memory with FDC_DOSE_TO_HOST.
+ */
+int fdc_run(fdc_ctx *ctx, const fdc_beamlet *b, uint32_t n_beamlets,
+            uint64_t first_proton, uint64_t n_protons, uint64_t proton_stride,
+            uint64_t seed, uint32_t flags, float *dose_gy);
+
+/* Copy out the raw fixed-point grid (nx*ny*nz u64, quanta of 2^-24 MeV). */
+int fdc_get_edep_fixed(fdc_ctx *ctx, uint64_t *grid_out, int is_device_ptr);
+
+/* Overwrite the raw fixed-point grid, e.g. with the sum over GPUs after an integer all-reduce (the
+ * paper's "absorbed dose from both threads was combined"); counters are unchanged. */
+int fdc_set_edep_fixed(fdc_ctx *ctx, const uint64_t *grid_in, int is_device_ptr);
+
+/* Counters accumulated since creation / the last fdc_reset (host struct; synchronises). */
+int fdc_get_stats(fdc_ctx *ctx, fdc_stats *out);
+
+/* Zero the grid and the counters. */
+int fdc_reset(fdc_ctx *ctx);
+
+void fdc_destroy(fdc_ctx *ctx);
+
+const char *fdc_strerror(int code);
+const char *fdc_last_error(const fdc_ctx *ctx);      /* text of the last FDC_ECUDA / FDC_EINVAL */
+
+/* Device time in milliseconds of the kernels of the most recent fdc_run, measured with CUDA events
+ * on the context's stream: [0] whole call on the device, [1] transport+deposit kernels only,
+ * [2] sampling-key + sort kernels, [3] Gy kernel.  launches = kernels launched by that call.
+ * Synchronises the stream. */
+int fdc_last_timing(fdc_ctx *ctx, float ms[4], uint32_t *launches);
+
+/*
+ * Roofline denominator: measured throughput of 64-bit reductions (`red.global.add.u64`, the
+ * deposit instruction) over a buffer of footprint_bytes on `device`: n_ops operations from a
+ * saturating grid, addresses from an integer hash of the operation index (the footprint is rounded
+ * down to a power of two).  mode 0: uniform over the footprint; 1: the 32 lanes of a warp fall in one 32-byte sector group (4 distinct words);
+ * 2: all lanes of a warp hit one word.  Returns operations per second in *ops_per_s.
+ */
+int fdc_peak_red_u64(int device, uint64_t footprint_bytes, uint64_t n_ops, int mode, double *ops_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDC_H */

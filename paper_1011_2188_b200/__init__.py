@@ -1,0 +1,202 @@
+"""Thin ctypes binding over the C-ABI of include/fdc.h (libfdc.so, CUDA kernels for sm_100a).
+
+Same names as the C functions; argument marshalling only -- every stage of the path (sampling,
+track selection, transport, deposit, Gy conversion) runs in the library's kernels.  torch is used
+for device memory and the stream, nothing else.  There is NO CPU fallback: a missing library or
+a non-sm_100 device raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfdc.so")
+
+FDC_RANDOM_AZIMUTH = 1
+FDC_DOSE_TO_HOST = 2
+FDC_NO_SORT = 4
+FDC_NO_AGGREGATE = 8
+
+FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH = 0, -1, -2, -3, -4, -5, -6
+
+EXPORTS = ["fdc_create", "fdc_load_tracks", "fdc_run", "fdc_get_edep_fixed", "fdc_set_edep_fixed", "fdc_get_stats", "fdc_reset",
+           "fdc_destroy", "fdc_strerror", "fdc_last_error", "fdc_last_timing", "fdc_peak_red_u64"]
+
+BEAMLET_DTYPE = np.dtype([("origin", "<f4", 3), ("e1", "<f4", 3), ("e2", "<f4", 3), ("dir", "<f4", 3),
+                          ("energy_mev", "<f4"), ("spot_u_mm", "<f4"), ("spot_v_mm", "<f4"),
+                          ("sigma_mm", "<f4"), ("n_protons", "<u8")], align=True)
+KNOT_DTYPE = np.dtype([("hu", "<f4"), ("density_g_cc", "<f4"), ("mass_spr", "<f4"), ("mass_scpr", "<f4")], align=True)
+
+
+class FdcError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("fdc error %d: %s" % (code, msg))
+        self.code = code
+
+
+class _TrackDB(ctypes.Structure):
+    _fields_ = [("dx", ctypes.c_void_p), ("dy", ctypes.c_void_p), ("dz", ctypes.c_void_p), ("dE", ctypes.c_void_p),
+                ("E", ctypes.c_void_p), ("n_steps", ctypes.c_uint64), ("track_off", ctypes.c_void_p),
+                ("n_tracks", ctypes.c_uint32), ("bin_first", ctypes.c_void_p), ("n_bins", ctypes.c_uint32),
+                ("e_min_mev", ctypes.c_float), ("e_bin_mev", ctypes.c_float)]
+
+
+class _Stats(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_uint64) for n in ("protons", "proton_steps", "deposits", "missed", "escaped", "stopped",
+                                               "grid_sum", "q_replayed", "q_escaped")]
+
+
+_lib = None
+
+
+def lib():
+    """Load libfdc.so (built in-tree by build.py / __graft_entry__.build()).  Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("%s not found: build it with `python -m paper_1011_2188_b200.build` "
+                              "(there is no CPU fallback)" % LIB_PATH)
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i32, u32, u64, f32 = ctypes.c_void_p, ctypes.c_int, ctypes.c_uint32, ctypes.c_uint64, ctypes.c_float
+        L.fdc_create.restype = i32
+        L.fdc_create.argtypes = [ctypes.POINTER(vp), i32, vp, vp, i32, i32, i32, f32, f32, f32, vp, i32, i32]
+        L.fdc_load_tracks.restype = i32
+        L.fdc_load_tracks.argtypes = [vp, ctypes.POINTER(_TrackDB), i32]
+        L.fdc_run.restype = i32
+        L.fdc_run.argtypes = [vp, vp, u32, u64, u64, u64, u64, u32, vp]
+        L.fdc_get_edep_fixed.restype = i32
+        L.fdc_get_edep_fixed.argtypes = [vp, vp, i32]
+        L.fdc_set_edep_fixed.restype = i32
+        L.fdc_set_edep_fixed.argtypes = [vp, vp, i32]
+        L.fdc_get_stats.restype = i32
+        L.fdc_get_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
+        L.fdc_reset.restype = i32
+        L.fdc_reset.argtypes = [vp]
+        L.fdc_destroy.restype = None
+        L.fdc_destroy.argtypes = [vp]
+        L.fdc_strerror.restype = ctypes.c_char_p
+        L.fdc_strerror.argtypes = [i32]
+        L.fdc_last_error.restype = ctypes.c_char_p
+        L.fdc_last_error.argtypes = [vp]
+        L.fdc_last_timing.restype = i32
+        L.fdc_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float * 4), ctypes.POINTER(u32)]
+        L.fdc_peak_red_u64.restype = i32
+        L.fdc_peak_red_u64.argtypes = [i32, u64, u64, i32, ctypes.POINTER(ctypes.c_double)]
+        _lib = L
+    return _lib
+
+
+def _ptr(x):
+    """Pointer of a numpy array (host) or torch tensor (host or device); None -> NULL."""
+    if x is None:
+        return None
+    if isinstance(x, np.ndarray):
+        assert x.flags["C_CONTIGUOUS"]
+        return ctypes.c_void_p(x.ctypes.data)
+    assert x.is_contiguous()
+    return ctypes.c_void_p(x.data_ptr())
+
+
+def _is_device(x):
+    return (not isinstance(x, np.ndarray)) and x.is_cuda
+
+
+def fdc_peak_red_u64(device: int, footprint_bytes: int, n_ops: int, mode: int = 0) -> float:
+    out = ctypes.c_double(0.0)
+    rc = lib().fdc_peak_red_u64(device, footprint_bytes, n_ops, mode, ctypes.byref(out))
+    if rc != 0:
+        raise FdcError(rc, lib().fdc_strerror(rc).decode())
+    return out.value
+
+
+class Fdc:
+    """One fdc_ctx.  Methods mirror the C-ABI one to one."""
+
+    def __init__(self, hu, spacing, table, device: int = 0, stream=None):
+        """fdc_create.  hu: int16 [nz,ny,nx] numpy array (copied) or CUDA torch tensor (borrowed)."""
+        import torch
+        self._lib = lib()
+        self._h = ctypes.c_void_p(None)
+        self._keep = []
+        nz, ny, nx = hu.shape
+        self.shape = (nz, ny, nx)
+        self.device = device
+        self._torch = torch
+        if stream is None:
+            stream = torch.cuda.current_stream(device)
+        self.stream = stream
+        table = np.ascontiguousarray(table, dtype=KNOT_DTYPE)
+        if _is_device(hu):
+            self._keep.append(hu)
+        h = ctypes.c_void_p(None)
+        rc = self._lib.fdc_create(ctypes.byref(h), device, ctypes.c_void_p(stream.cuda_stream), _ptr(hu), nx, ny, nz,
+                                  float(spacing[0]), float(spacing[1]), float(spacing[2]), _ptr(table), len(table),
+                                  1 if _is_device(hu) else 0)
+        if rc != 0:
+            raise FdcError(rc, self._lib.fdc_strerror(rc).decode())
+        self._h = h
+
+    def _check(self, rc):
+        if rc != 0:
+            raise FdcError(rc, "%s: %s" % (self._lib.fdc_strerror(rc).decode(), self._lib.fdc_last_error(self._h).decode()))
+
+    def fdc_load_tracks(self, dx, dy, dz, dE, E, track_off, bin_first, e_min, e_bin):
+        """Step arrays: all numpy (host) or all CUDA torch tensors; offsets: numpy."""
+        dev = _is_device(dx)
+        assert all(_is_device(a) == dev for a in (dy, dz, dE, E))
+        track_off = np.ascontiguousarray(track_off, dtype=np.uint64)
+        bin_first = np.ascontiguousarray(bin_first, dtype=np.uint32)
+        n = int(dx.shape[0])
+        db = _TrackDB(_ptr(dx).value, _ptr(dy).value, _ptr(dz).value, _ptr(dE).value, _ptr(E).value, n,
+                      track_off.ctypes.data, len(track_off) - 1, bin_first.ctypes.data, len(bin_first) - 1,
+                      float(e_min), float(e_bin))
+        self._check(self._lib.fdc_load_tracks(self._h, ctypes.byref(db), 1 if dev else 0))
+
+    def fdc_run(self, beamlets, first_proton, n_protons, proton_stride, seed, flags=FDC_RANDOM_AZIMUTH, dose_gy=None):
+        """dose_gy: None, a CUDA float32 tensor [nz,ny,nx], or a host numpy/pinned-torch float32 array."""
+        bl = np.ascontiguousarray(beamlets, dtype=BEAMLET_DTYPE)
+        flags = int(flags) & ~FDC_DOSE_TO_HOST
+        if dose_gy is not None and not _is_device(dose_gy):
+            flags |= FDC_DOSE_TO_HOST
+        self._check(self._lib.fdc_run(self._h, _ptr(bl), len(bl), int(first_proton), int(n_protons), int(proton_stride),
+                                      int(seed), flags, _ptr(dose_gy)))
+
+    def fdc_get_edep_fixed(self, out=None):
+        """Raw grid; out: CUDA int64 tensor, or None -> new host numpy uint64 [nz,ny,nx]."""
+        if out is None:
+            out = np.empty(self.shape, dtype=np.uint64)
+        self._check(self._lib.fdc_get_edep_fixed(self._h, _ptr(out), 1 if _is_device(out) else 0))
+        return out
+
+    def fdc_set_edep_fixed(self, grid):
+        """Overwrite the raw grid from a CUDA int64 tensor or a host numpy uint64 array."""
+        self._check(self._lib.fdc_set_edep_fixed(self._h, _ptr(grid), 1 if _is_device(grid) else 0))
+
+    def fdc_get_stats(self) -> dict:
+        s = _Stats()
+        self._check(self._lib.fdc_get_stats(self._h, ctypes.byref(s)))
+        return {n: int(getattr(s, n)) for n, _ in s._fields_}
+
+    def fdc_reset(self):
+        self._check(self._lib.fdc_reset(self._h))
+
+    def fdc_last_timing(self) -> dict:
+        ms = (ctypes.c_float * 4)()
+        n = ctypes.c_uint32(0)
+        self._check(self._lib.fdc_last_timing(self._h, ctypes.byref(ms), ctypes.byref(n)))
+        return {"total_ms": ms[0], "transport_ms": ms[1], "sort_ms": ms[2], "gy_ms": ms[3], "launches": int(n.value)}
+
+    def fdc_destroy(self):
+        if self._h:
+            self._lib.fdc_destroy(self._h)
+            self._h = ctypes.c_void_p(None)
+            self._keep = []
+
+    def __del__(self):
+        try:
+            self.fdc_destroy()
+        except Exception:
+            pass

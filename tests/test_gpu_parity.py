@@ -1,0 +1,239 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the oracle, element by element on the same
+seeded inputs.  Bar (north_star): the u64 fixed-point grid is BIT-EXACT; the Gy grid
+is then identical too (same f64 formula); every counter of fdc_stats equals the oracle's."""
+import numpy as np
+import pytest
+
+import fdc_inputs as fi
+
+pytestmark = pytest.mark.gpu
+
+STAT_KEYS = ("protons", "proton_steps", "deposits", "missed", "escaped", "stopped", "grid_sum", "q_replayed", "q_escaped")
+
+
+@pytest.fixture(scope="module")
+def fdc():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    import paper_1011_2188_b200 as m
+    m.lib()                       # fails loudly if libfdc.so is missing: there is no fallback
+    return m
+
+
+def make_ctx(fdc, w, device_arrays=False):
+    import torch
+    if device_arrays:
+        hu = torch.from_numpy(w.phantom.hu).cuda()
+        ctx = fdc.Fdc(hu, w.phantom.spacing, w.table)
+        t = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (w.db.dx, w.db.dy, w.db.dz, w.db.dE, w.db.E)]
+        ctx.fdc_load_tracks(*t, w.db.track_off, w.db.bin_first, w.db.e_min, w.db.e_bin)
+    else:
+        ctx = fdc.Fdc(np.ascontiguousarray(w.phantom.hu), w.phantom.spacing, w.table)
+        ctx.fdc_load_tracks(*[np.ascontiguousarray(a) for a in (w.db.dx, w.db.dy, w.db.dz, w.db.dE, w.db.E)],
+                            w.db.track_off, w.db.bin_first, w.db.e_min, w.db.e_bin)
+    return ctx
+
+
+def check_against_oracle(fdc, w, ctx=None, flags=1, first=0, n=None, stride=1, seed=None):
+    import oracle
+    seed = w.seed if seed is None else seed
+    n = w.n_protons if n is None else n
+    own = ctx is None
+    if own:
+        ctx = make_ctx(fdc, w)
+    ctx.fdc_reset()
+    dose = np.zeros(w.phantom.hu.shape, dtype=np.float32)
+    ctx.fdc_run(w.beamlets, first, n, stride, seed, flags=flags, dose_gy=dose)
+    g = ctx.fdc_get_edep_fixed()
+    st = ctx.fdc_get_stats()
+    og, ost = oracle.run(w.phantom, w.table, w.db, w.beamlets, seed, first=first, n=n, stride=stride, flags=flags & 1)
+    assert np.array_equal(g, og), "fixed-point grid differs: %d voxels, sum %d vs %d" % (
+        int((g != og).sum()), int(g.sum(dtype=np.uint64)), int(og.sum(dtype=np.uint64)))
+    for k in STAT_KEYS:
+        assert st[k] == ost[k], (k, st[k], ost[k])
+    assert st["grid_sum"] + st["q_escaped"] == st["q_replayed"]
+    assert np.array_equal(dose, oracle.to_gy(og, w.phantom, w.table))
+    if own:
+        ctx.fdc_destroy()
+    return g, st
+
+
+# ------------------------------------------------------------------ reduced-size configs, every element
+def test_config1_reduced(fdc, wl1_small):
+    check_against_oracle(fdc, wl1_small)
+
+
+def test_config2_reduced(fdc, wl2_small):
+    g, st = check_against_oracle(fdc, wl2_small)
+    assert st["escaped"] == wl2_small.n_protons
+
+
+def test_config3_reduced(fdc, wl3_small):
+    g, st = check_against_oracle(fdc, wl3_small)
+    assert st["deposits"] > 10 * st["proton_steps"] / 8          # air columns: many voxels per step
+
+
+def test_flags_and_ranges(fdc, wl3_small):
+    w = wl3_small
+    ctx = make_ctx(fdc, w, device_arrays=True)
+    g_sorted, _ = check_against_oracle(fdc, w, ctx)
+    g_nosort, _ = check_against_oracle(fdc, w, ctx, flags=1 | fdc.FDC_NO_SORT)
+    g_noagg, _ = check_against_oracle(fdc, w, ctx, flags=1 | fdc.FDC_NO_AGGREGATE)
+    assert np.array_equal(g_sorted, g_nosort) and np.array_equal(g_sorted, g_noagg)
+    check_against_oracle(fdc, w, ctx, flags=0)                                   # azimuth off
+    check_against_oracle(fdc, w, ctx, first=7, n=300, stride=13)                 # strided subset
+    check_against_oracle(fdc, w, ctx, first=4000, n=704)                         # tail range
+    check_against_oracle(fdc, w, ctx, seed=2 ** 40 + 12345)                      # 64-bit seed
+    # accumulation: run(0..a) + run(a..N) == run(0..N), bit for bit (P7)
+    ctx.fdc_reset()
+    ctx.fdc_run(w.beamlets, 1000, w.n_protons - 1000, 1, w.seed)
+    ctx.fdc_run(w.beamlets, 0, 1000, 1, w.seed)
+    assert np.array_equal(ctx.fdc_get_edep_fixed(), g_sorted)
+    # n_protons = 0 is a no-op
+    ctx.fdc_reset()
+    ctx.fdc_run(w.beamlets, 0, 0, 1, w.seed)
+    assert ctx.fdc_get_stats()["protons"] == 0 and not ctx.fdc_get_edep_fixed().any()
+    # device output buffers
+    import torch
+    ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed)
+    gd = torch.zeros(w.phantom.hu.shape, dtype=torch.int64, device="cuda")
+    ctx.fdc_get_edep_fixed(gd)
+    dd = torch.zeros(w.phantom.hu.shape, dtype=torch.float32, device="cuda")
+    ctx.fdc_run(w.beamlets, 0, 0, 1, w.seed, dose_gy=dd)
+    torch.cuda.synchronize()
+    assert np.array_equal(gd.cpu().numpy().view(np.uint64), g_sorted)
+    import oracle
+    assert np.array_equal(dd.cpu().numpy(), oracle.to_gy(g_sorted, w.phantom, w.table))
+    ctx.fdc_destroy()
+
+
+def test_hand_made_cases(fdc):
+    """Closed-form inputs of tests/test_oracle_pins.py: straight, split, half density, interface,
+    oblique, angle scaling, zero-length step, escape, miss -- all bit-exact against the oracle."""
+    from test_oracle_pins import hand_db, table_uniform, uniform_phantom
+    cases = []
+    ph = uniform_phantom(16, 1.0)
+    cases.append((ph, table_uniform(1.0), hand_db([[(0, 0, 1.0, (k + 1) / 8.0) for k in range(10)]]),
+                  fi.single_beamlet((5.5, 6.5, 0.0), 100.0, 0.0, 3), 1))
+    cases.append((ph, table_uniform(1.0), hand_db([[(0, 0, 1.0, 1.0 + k / 4.0) for k in range(6)]]),
+                  fi.single_beamlet((5.5, 6.5, 0.25), 100.0, 0.0, 1), 1))
+    cases.append((ph, table_uniform(0.5), hand_db([[(0, 0, 1.0, 1.0) for _ in range(4)]]),
+                  fi.single_beamlet((5.5, 6.5, 0.0), 100.0, 0.0, 1), 1))
+    cases.append((ph, table_uniform(1.0), hand_db([[(0, 0, 4.5, 4.5)]]),
+                  fi.single_beamlet((0.4, 4.5, 0.0), 100.0, 0.0, 1, e1=(0.8, 0, -0.6), e2=(0, 1, 0), d=(0.6, 0, 0.8)), 0))
+    tau = 0.05; n1 = float(np.hypot(1.0, tau)); u1 = (tau / n1, 0.0, 1.0 / n1)
+    cases.append((uniform_phantom(32, 1.0), table_uniform(1.0, 1.0, 2.25),
+                  hand_db([[(0, 0, 1.0, 1.0), u1 + (1.0,), u1 + (1.0,), (0.1, 0.2, 0.9, 1.5)]]),
+                  fi.single_beamlet((16.5, 16.5, 0.0), 100.0, 2.0, 50), 1))
+    cases.append((uniform_phantom(8, 1.0), table_uniform(1.0), hand_db([[(0, 0, 1.0, 1.0), (0, 0, 0.0, 2.0), (0, 0, 1.0, 1.0)]]),
+                  fi.single_beamlet((3.5, 3.5, 0.0), 100.0, 0.0, 2), 1))
+    cases.append((uniform_phantom(8, 1.0), table_uniform(1.0), hand_db([[(0, 0, 1.0, 0.5 + 0.125 * k) for k in range(12)]]),
+                  fi.single_beamlet((3.5, 3.5, 0.25), 100.0, 0.0, 1), 1))
+    cases.append((uniform_phantom(8, 1.0), table_uniform(1.0), hand_db([[(0, 0, 1.0, 1.0)]]),
+                  fi.single_beamlet((30.0, 3.5, -5.0), 100.0, 0.0, 4), 1))          # misses the grid
+    cases.append((uniform_phantom(8, 1.0), table_uniform(1.0), hand_db([[(0, 0, 1.0, 1.0)]]),
+                  fi.single_beamlet((3.5, 3.5, 0.0), 10.0, 0.0, 2), 1))             # replays nothing
+    ph_if = fi.make_phantom("uniform", (8, 8, 16), (1.0, 1.0, 0.5)); ph_if.hu[3:, :, :] = -500
+    tab_if = np.array([(-500.0, 0.5, 1.0, 1.0), (0.0, 1.0, 1.0, 1.0)], dtype=fi.KNOT_DTYPE)
+    cases.append((ph_if, tab_if, hand_db([[(0, 0, 1.0, 1.0), (0, 0, 1.0, 2.0)]]), fi.single_beamlet((3.5, 3.5, 0.0), 100.0, 0.0, 1), 1))
+    for ph, tab, db, bl, flags in cases:
+        w = fi.Workload("hand", ph, tab, db, bl, int(bl["n_protons"].sum()), 5)
+        check_against_oracle(fdc, w, flags=flags)
+
+
+def test_errors(fdc, wl2_small):
+    w = wl2_small
+    hu = np.ascontiguousarray(w.phantom.hu)
+    ctx = fdc.Fdc(hu, w.phantom.spacing, w.table)
+    with pytest.raises(fdc.FdcError) as e:
+        ctx.fdc_run(w.beamlets, 0, 10, 1, 1)
+    assert e.value.code == fdc.FDC_ENOTRACKS
+    arrs = [np.ascontiguousarray(a) for a in (w.db.dx, w.db.dy, w.db.dz, w.db.dE, w.db.E)]
+    bad = [a.copy() for a in arrs]; bad[4][5] = 1e9                                  # E increases within a track
+    with pytest.raises(fdc.FdcError) as e:
+        ctx.fdc_load_tracks(*bad, w.db.track_off, w.db.bin_first, w.db.e_min, w.db.e_bin)
+    assert e.value.code == fdc.FDC_EINVAL
+    bad = [a.copy() for a in arrs]; bad[3][7] = -1.0                                 # negative dE
+    with pytest.raises(fdc.FdcError) as e:
+        ctx.fdc_load_tracks(*bad, w.db.track_off, w.db.bin_first, w.db.e_min, w.db.e_bin)
+    assert e.value.code == fdc.FDC_EINVAL
+    off = w.db.track_off.copy(); off[-1] += 1
+    with pytest.raises(fdc.FdcError) as e:
+        ctx.fdc_load_tracks(*arrs, off, w.db.bin_first, w.db.e_min, w.db.e_bin)
+    assert e.value.code == fdc.FDC_EINVAL
+    ctx.fdc_load_tracks(*arrs, w.db.track_off, w.db.bin_first, w.db.e_min, w.db.e_bin)
+    for kw, code in [(dict(proton_stride=0), fdc.FDC_EINVAL), (dict(first_proton=w.n_protons), fdc.FDC_EINVAL),
+                     (dict(n_protons=w.n_protons + 1), fdc.FDC_EINVAL), (dict(first_proton=5, n_protons=w.n_protons), fdc.FDC_EINVAL)]:
+        a = dict(first_proton=0, n_protons=10, proton_stride=1); a.update(kw)
+        with pytest.raises(fdc.FdcError) as e:
+            ctx.fdc_run(w.beamlets, a["first_proton"], a["n_protons"], a["proton_stride"], 1)
+        assert e.value.code == code
+    bl = w.beamlets.copy(); bl["energy_mev"] = 170.0                                 # above the top bin
+    with pytest.raises(fdc.FdcError) as e:
+        ctx.fdc_run(bl, 0, 10, 1, 1)
+    assert e.value.code == fdc.FDC_ERANGE
+    bl = w.beamlets.copy(); bl["energy_mev"] = 145.0                                 # bin exists but lazily left empty
+    with pytest.raises(fdc.FdcError) as e:
+        ctx.fdc_run(bl, 0, 10, 1, 1)
+    assert e.value.code == fdc.FDC_ERANGE
+    bl = w.beamlets.copy(); bl["dir"] = (0.0, 0.1, 1.0)                              # not a unit vector
+    with pytest.raises(fdc.FdcError) as e:
+        ctx.fdc_run(bl, 0, 10, 1, 1)
+    assert e.value.code == fdc.FDC_EINVAL
+    assert not ctx.fdc_get_edep_fixed().any()                                         # failures left no partial state
+    ctx.fdc_destroy()
+    with pytest.raises(fdc.FdcError) as e:
+        fdc.Fdc(hu, (1.0, 0.0, 1.0), w.table)
+    assert e.value.code == fdc.FDC_EINVAL
+    tab = w.table.copy(); tab["hu"][2] = tab["hu"][1]
+    with pytest.raises(fdc.FdcError) as e:
+        fdc.Fdc(hu, w.phantom.spacing, tab)
+    assert e.value.code == fdc.FDC_EINVAL
+
+
+def test_hu_outside_table_is_clamped(fdc):
+    from test_oracle_pins import hand_db
+    ph = fi.make_phantom("uniform", (8, 8, 8), (1.0, 1.0, 1.0))
+    ph.hu[:4] = -2000; ph.hu[4:] = 32000
+    db = hand_db([[(0, 0, 1.0, 1.0)] * 12])
+    w = fi.Workload("clamp", ph, fi.material_table("config2"), db, fi.single_beamlet((3.5, 3.5, 7.9), 100.0, 0.0, 3, e1=(0, 1, 0), e2=(1, 0, 0), d=(0, 0, -1)), 3, 9)
+    check_against_oracle(fdc, w)
+
+
+# ------------------------------------------------------------------ full sizes, in bench.py's launch configuration
+def test_config1_full_bit_exact(fdc):
+    w = fi.workload(1)
+    g, st = check_against_oracle(fdc, w)
+    assert st["protons"] == 100_000 and st["escaped"] == 0
+    assert abs(st["grid_sum"] / 2 ** 24 / 1e5 - 100.0) < 1e-4
+
+
+def test_config2_full_bit_exact(fdc):
+    """BASELINE.json configs[1] at full size (1e6 protons, 1e4 tracks in the 150 MeV bin): the
+    workload bench.py times.  The oracle needs some tens of seconds for it."""
+    w = fi.workload(2)
+    g, st = check_against_oracle(fdc, w)
+    assert st["protons"] == 1_000_000
+
+
+@pytest.mark.parametrize("cfg,n_sub", [(3, 100_000), (4, 100_000)])
+def test_config34_full_db_strided_subset(fdc, cfg, n_sub):
+    """Configs 3/4 with the full-size database and plan; the oracle runs every K-th proton (so every
+    field, layer and spot is represented) and the GPU runs the same subset, word for word.  Then the
+    GPU runs the whole plan and is checked by properties that hold at any size: conservation, and
+    full == sum of two halves."""
+    w = fi.workload(cfg)
+    ctx = make_ctx(fdc, w)
+    K = w.n_protons // n_sub
+    check_against_oracle(fdc, w, ctx, first=K // 2, n=n_sub, stride=K)
+    if cfg == 3:
+        ctx.fdc_reset()
+        ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed)
+        g = ctx.fdc_get_edep_fixed(); st = ctx.fdc_get_stats()
+        assert st["protons"] == w.n_protons == st["missed"] + st["escaped"] + st["stopped"]
+        assert st["grid_sum"] + st["q_escaped"] == st["q_replayed"] and st["grid_sum"] == int(g.sum(dtype=np.uint64))
+        ctx.fdc_reset()
+        ctx.fdc_run(w.beamlets, w.n_protons // 2, w.n_protons - w.n_protons // 2, 1, w.seed)
+        ctx.fdc_run(w.beamlets, 0, w.n_protons // 2, 1, w.seed)
+        assert np.array_equal(ctx.fdc_get_edep_fixed(), g)
+    ctx.fdc_destroy()
