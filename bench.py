@@ -26,7 +26,6 @@ from __future__ import annotations
 import argparse
 import json
 import os
-import subprocess
 import sys
 import threading
 import time
@@ -50,50 +49,59 @@ def _peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks + throttle reasons sampled every 200 ms while the timed region runs."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """SM clock + throttle reasons sampled through NVML every few ms while the timed region runs
+    (nvidia-smi -lms cannot sample a region that lasts tens of milliseconds)."""
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
 
-    def __init__(self, index):
-        self.index, self.proc, self.lines = index, None, []
+    def __init__(self, index, period_s=0.004):
+        self.index, self.period, self.samples, self.stop_flag, self.t, self.err = index, period_s, [], False, None, None
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "200"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=self._read, daemon=True)
-            self.t.start()
-        except OSError:
-            self.proc = None
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:                                    # CUDA_VISIBLE_DEVICES may renumber: go by UUID
+                import torch
+                self.h = pynvml.nvmlDeviceGetHandleByUUID("GPU-" + str(torch.cuda.get_device_properties(self.index).uuid))
+            except Exception:                       # noqa: BLE001
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:                      # noqa: BLE001 -- reported in the JSON line
+            self.err = "nvml unavailable: %s" % e
+            return
+        self.t = threading.Thread(target=self._poll, daemon=True)
+        self.t.start()
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.lines.append(line.strip())
+    def _poll(self):
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                try:
+                    rs = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:                   # noqa: BLE001 -- older binding name
+                    rs = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                self.samples.append((float(mhz), int(rs), pw))
+            except Exception as e:                  # noqa: BLE001
+                self.err = str(e)
+                break
+            time.sleep(self.period)
 
     def stop(self):
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except subprocess.TimeoutExpired:
-            self.proc.kill()
-        sm, mx, pw, reasons = [], [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.lines:
-            f = [x.strip() for x in ln.split(",")]
-            if len(f) < 7:
-                continue
-            try:
-                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
-            except ValueError:
-                continue
-            for n, v in zip(names, f[3:7]):
-                if v.lower() == "active":
-                    reasons.add(n)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+        self.stop_flag = True
+        if self.t is not None:
+            self.t.join(timeout=2)
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "samples": 0, "reasons": [self.err or "no samples"]}
+        sm = [s[0] for s in self.samples]
+        bits = 0
+        for s in self.samples:
+            bits |= s[1]
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": self.max_mhz, "sm_mhz_min": min(sm), "sm_mhz_peak": max(sm),
+                "power_w_max": max(s[2] for s in self.samples), "samples": len(sm),
+                "reasons": sorted(n for b, n in self.REASONS.items() if bits & b)}
 
 
 def make_workload(cfg, gpus):
@@ -235,7 +243,7 @@ def run_fdc(args):
 
     # cold variant: phantom + database from host memory every step (N = 1 only; bounded to 3 steps)
     e2e_cold = None
-    if world == 1 and rank == 0:
+    if world == 1 and rank == 0 and not args.no_cold:
         hu_h = np.ascontiguousarray(w.phantom.hu)
         cold_ms, ncold = 0.0, min(3, args.steps)
         for it in range(1 + ncold):
@@ -323,13 +331,14 @@ def run_fdc(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="fdc", choices=["fdc", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[C-1]; 2 is the headline single-GPU workload")
-    ap.add_argument("--cpu-sample", type=int, default=500_000, help="protons of the strided subset the oracle is timed on")
+    ap.add_argument("--cpu-sample", type=int, default=1_000_000, help="protons of the strided subset the oracle is timed on")
     ap.add_argument("--ref-sample", type=int, default=100_000, help="--impl reference: protons per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cold", action="store_true", help="skip the e2e_cold leg (context + database re-created from host memory)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "fdc":
         print("note: warmup < 3 breaks the timing rules; use for smoke runs only", file=sys.stderr)
