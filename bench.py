@@ -120,7 +120,7 @@ def run_reference(args):
         return 0
     import oracle
     w, per_rank = make_workload(args.config, 1)
-    n_sub = args.ref_sample
+    n_sub = min(args.ref_sample, w.n_protons)
     K = max(1, w.n_protons // n_sub)
     times, steps, deps = [], 0, 0
     for it in range(args.warmup + args.steps):
@@ -297,7 +297,7 @@ def run_fdc(args):
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
             import oracle
-            n_sub = args.cpu_sample
+            n_sub = min(args.cpu_sample, w.n_protons)
             K = max(1, w.n_protons // n_sub)
             t0 = time.perf_counter()
             og, ost = oracle.run(w.phantom, w.table, w.db, w.beamlets, w.seed, first=0, n=n_sub, stride=K)

@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfdc.so")
+LIB_PATH = os.environ.get("FDC_LIB") or os.path.join(_HERE, "libfdc.so")      # FDC_LIB: another build of the same library
 
 FDC_RANDOM_AZIMUTH = 1
 FDC_DOSE_TO_HOST = 2
