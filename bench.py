@@ -272,7 +272,12 @@ def run_fdc(args):
         n_vox = int(np.prod(w.phantom.hu.shape))
         # roofline of the dominant kernel (k_transport), rank 0's launches, live CUDA-event durations
         tr_ms = float(np.mean([k["transport_ms"] for k in ktimes]))
-        red_peak = fdc.fdc_peak_red_u64(local, n_vox * 8, 1 << 30, 0)
+        # denominators: u64 red rate, uniform random addresses, (i) over an L2-resident buffer and (ii) over a
+        # buffer the size of this grid.  (i) >= (ii); the kernel's deposits are spatially clustered, so on a
+        # grid larger than L2 it can beat (ii) -- the roofline therefore uses (i), the harder ceiling.
+        red_l2 = fdc.fdc_peak_red_u64(local, min(n_vox * 8, 64 << 20), 1 << 30, 0)
+        red_fp = red_l2 if n_vox * 8 <= (64 << 20) else fdc.fdc_peak_red_u64(local, n_vox * 8, 1 << 28, 0)
+        red_peak = max(red_l2, red_fp)
         t_track = st["proton_steps"] * STEP_RECORD_BYTES / (hbm_gbs * 1e9)
         t_atomic = st["deposits"] / red_peak
         bound_atomic = t_atomic >= t_track
@@ -286,8 +291,12 @@ def run_fdc(args):
                 "t_track_ms": t_track * 1e3, "t_atomic_ms": t_atomic * 1e3,
                 "hbm": {"achieved_gbs": st["proton_steps"] * STEP_RECORD_BYTES / (tr_ms * 1e-3) / 1e9, "peak_gbs": hbm_gbs, "peak_source": peak_src},
                 "l2_atomic": {"achieved_gred_s": st["deposits"] / (tr_ms * 1e-3) / 1e9, "peak_gred_s": red_peak / 1e9,
-                              "peak_source": "fdc_peak_red_u64: u64 red, uniform random addresses over the grid's %d MiB, measured in this run" % (n_vox * 8 >> 20)},
-                "algorithmic": {"proton_steps": st["proton_steps"], "deposits": st["deposits"], "bytes_per_step": STEP_RECORD_BYTES}}
+                              "peak_at_grid_footprint_gred_s": red_fp / 1e9, "grid_mib": n_vox * 8 >> 20,
+                              "peak_source": "fdc_peak_red_u64 measured in this run: u64 red, uniform random addresses over min(grid, 64 MiB) "
+                                             "(L2-resident); peak_at_grid_footprint is the same over the whole grid"},
+                "algorithmic": {"proton_steps": st["proton_steps"], "deposits": st["deposits"], "bytes_per_step": STEP_RECORD_BYTES,
+                                "note": "deposits = non-zero (step, voxel) shares (R8); the kernel merges the shares one proton leaves in "
+                                        "one voxel into a single red, so it issues fewer reds than deposits"}}
         traffic_file = os.path.join(ROOT, "profiles", "traffic_config%d.json" % args.config)
         if os.path.exists(traffic_file):
             with open(traffic_file) as f:
