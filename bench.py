@@ -297,10 +297,13 @@ def run_fdc(args):
                 "algorithmic": {"proton_steps": st["proton_steps"], "deposits": st["deposits"], "bytes_per_step": STEP_RECORD_BYTES,
                                 "note": "deposits = non-zero (step, voxel) shares (R8); the kernel merges the shares one proton leaves in "
                                         "one voxel into a single red, so it issues fewer reds than deposits"}}
-        traffic_file = os.path.join(ROOT, "profiles", "traffic_config%d.json" % args.config)
+        traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")     # dram bytes of one ncu --set full capture, per launch
         if os.path.exists(traffic_file):
             with open(traffic_file) as f:
-                roof["traffic"] = json.load(f).get("dram_bytes_per_launch")
+                for line in f.read().splitlines()[1:]:
+                    c = line.split(",")
+                    if len(c) >= 2 and c[0].strip() == str(args.config):
+                        roof["traffic"] = float(c[1])
 
         # cpu baseline: the oracle on a bounded strided sample, this box's host cores
         cpu = None
