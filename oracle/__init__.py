@@ -126,6 +126,69 @@ def run(phantom, table, db, beamlets, seed, first=0, n=None, stride=1, flags=FLA
     return (grid, d, es) if (f64 and end_state) else (grid, d)
 
 
+def run_sq(phantom, table, db, beamlets, seed, first=0, n=None, stride=1, flags=FLAG_RANDOM_AZIMUTH, by_history=True):
+    """Whole path plus the sum-of-squares tallies (R10).  Returns (grid, sq_by_visit,
+    sq_by_history or None, stats): u64 grids [nz,ny,nx]; squares in quanta of 2^-32 MeV^2."""
+    if n is None:
+        n = int(beamlets["n_protons"].sum()) - first
+    grid = np.zeros(phantom.hu.shape, dtype=np.uint64)
+    sqv = np.zeros(phantom.hu.shape, dtype=np.uint64)
+    sqh = np.zeros(phantom.hu.shape, dtype=np.uint64) if by_history else None
+    st = StatsStruct()
+    a, keep = _common_args(phantom, table, db, beamlets)
+    a += _range_args(first, n, stride, seed, flags) + [_p(grid), _p(sqv), _p(sqh) if by_history else None, ctypes.byref(st)]
+    rc = lib().oracle_run_sq(*a)
+    if rc != 0:
+        raise RuntimeError("oracle_run_sq failed rc=%d" % rc)
+    d = st.as_dict()
+    d["grid_sum"] = int(grid.sum(dtype=np.uint64))
+    return grid, sqv, sqh, d
+
+
+# ---------------------------------------------------------------- PAPER.md §2.4, eq. (1), (2), mean uncertainty (numpy f64)
+E_QUANTUM = 2.0 ** -24      # MeV per unit of the energy grid
+SQ_QUANTUM = 2.0 ** -32     # MeV^2 per unit of the squares grid
+
+
+def sigma_history(grid, sq, n_histories):
+    """Eq. (2) (sums over all N primaries: reading A11), per voxel, of the MEAN energy per
+    history: sigma = sqrt(max(0, (sum e^2 / N - (sum e / N)^2)) / (N - 1)).  Returns (mean, sigma) in MeV."""
+    N = float(n_histories)
+    m1 = (grid.astype(np.float64) * E_QUANTUM) / N
+    m2 = (sq.astype(np.float64) * SQ_QUANTUM) / N
+    var = (m2 - m1 * m1) / (N - 1.0)
+    return m1, np.sqrt(np.maximum(var, 0.0))
+
+
+def sigma_batch(grids):
+    """Eq. (1): n independent batches D_i -> (mean, sqrt(sum (D_i - mean)^2 / (n (n - 1)))), MeV."""
+    n = len(grids)
+    D = [g.astype(np.float64) * E_QUANTUM for g in grids]
+    mean = D[0].copy()
+    for d in D[1:]:
+        mean = mean + d
+    mean = mean / float(n)
+    ss = np.zeros_like(mean)
+    for d in D:
+        ss = ss + (d - mean) * (d - mean)
+    return mean, np.sqrt(ss / float(n * (n - 1)))
+
+
+def mean_uncertainty(mean, sigma, rho):
+    """average of sigma/D over the voxels whose DOSE (energy / density; the voxel volume is
+    common) exceeds half the maximum dose.  Returns (value, number of voxels averaged)."""
+    dose = mean / rho.astype(np.float64)
+    sel = dose > 0.5 * dose.max()
+    rel = sigma[sel] / mean[sel]
+    return float(rel.mean()), int(sel.sum())
+
+
+def density(phantom, table):
+    """rho (f32) per voxel from the material LUT (R1)."""
+    rho, w, f = material_lut(table)
+    return rho[np.clip(phantom.hu.astype(np.int32), -1024, 3071) + 1024]
+
+
 def run_trace(phantom, table, db, beamlets, seed, first=0, n=1, stride=1, flags=FLAG_RANDOM_AZIMUTH, cap=1 << 20):
     """f32 run recording every deposit: returns grid, stats, (voxel, share, step), end_state[n,6]."""
     grid = np.zeros(phantom.hu.shape, dtype=np.uint64)

@@ -20,6 +20,9 @@
 #include <cmath>
 #include <cstring>
 #include <limits>
+#include <vector>
+#include <algorithm>
+#include <utility>
 
 namespace {
 
@@ -234,11 +237,34 @@ int start_proton(const Geometry &G, const TrackDB &db, const Beamlet *bl, uint32
 /* optional per-deposit trace for the bookkeeping pins (P8) */
 struct Trace { uint64_t *voxel; uint64_t *share; uint32_t *step; uint64_t cap, n; };
 
+/* R10: sum-of-squares tallies ("a second tallying array ... the sum of the squares of the
+ * deposited energy", eq. (2)).  Operand e' = e >> 8 (quanta of 2^-16 MeV, clamped to 2^32-1), tally
+ * += e'^2 (quanta of 2^-32 MeV^2).
+ *   by_history: e = ALL the energy history i left in the voxel -- eq. (2)'s D_i, the plain definition.
+ *   by_visit  : e = the energy left during one uninterrupted stay in the voxel (from entering it to
+ *               crossing out of it); equal to by_history unless a history re-enters a voxel (reading A23). */
+struct Squares { uint64_t *by_visit; uint64_t *by_history; };
+uint64_t sq_operand(uint64_t e) { uint64_t x = e >> 8; if (x > 0xffffffffull) x = 0xffffffffull; return x * x; }
+
 /* R7 + R8 for one proton */
 template <class T>
 void transport(const Geometry &G, const TrackDB &db, Start<T> &S, uint64_t *grid, Stats &st, Trace *tr,
-               T *end_state /* p[3], g[3] of the last step, may be null */)
+               T *end_state /* p[3], g[3] of the last step, may be null */, Squares *sq = nullptr)
 {
+    uint64_t visit_vox = 0, visit_sum = 0;                       /* R10 by_visit */
+    std::vector<std::pair<uint64_t, uint64_t>> history;          /* R10 by_history: every (voxel, share) of this proton */
+    auto end_visit = [&]() { if (sq && sq->by_visit && visit_sum) sq->by_visit[visit_vox] += sq_operand(visit_sum); visit_sum = 0; };
+    auto end_history = [&]() {
+        end_visit();
+        if (!(sq && sq->by_history)) return;
+        std::sort(history.begin(), history.end());
+        for (size_t a = 0; a < history.size();) {
+            size_t b = a; uint64_t e = 0;
+            while (b < history.size() && history[b].first == history[a].first) { e += history[b].second; ++b; }
+            sq->by_history[history[a].first] += sq_operand(e);
+            a = b;
+        }
+    };
     const T INF = std::numeric_limits<T>::infinity();
     const T TINY = (T)7.888609052210118e-31;     /* 2^-100 */
     T p[3] = {S.p[0], S.p[1], S.p[2]};
@@ -258,6 +284,7 @@ void transport(const Geometry &G, const TrackDB &db, Start<T> &S, uint64_t *grid
         auto deposit = [&](uint64_t v, uint64_t q) {
             if (q == 0) return;
             grid[v] += q; st.deposits++;
+            if (sq) { visit_vox = v; visit_sum += q; if (sq->by_history) history.push_back(std::make_pair(v, q)); }
             if (tr && tr->n < tr->cap) { tr->voxel[tr->n] = v; tr->share[tr->n] = q; tr->step[tr->n] = (uint32_t)(k - S.k0); tr->n++; }
         };
         const T d[3] = {(T)db.dx[k], (T)db.dy[k], (T)db.dz[k]};
@@ -348,6 +375,7 @@ void transport(const Geometry &G, const TrackDB &db, Start<T> &S, uint64_t *grid
             q_done = q_cum;
             tMax[ax] = tMax[ax] + tDelta[ax];
             iv[ax] += dirn[ax];
+            end_visit();                                         /* the proton has left the voxel */
             if (iv[ax] < 0 || iv[ax] >= G.n[ax]) { escaped = true; break; }
             vox = (uint64_t)iv[0] + (uint64_t)G.n[0] * ((uint64_t)iv[1] + (uint64_t)G.n[1] * (uint64_t)iv[2]);
         }
@@ -356,11 +384,13 @@ void transport(const Geometry &G, const TrackDB &db, Start<T> &S, uint64_t *grid
             st.q_escaped += Q - q_done;
             for (uint64_t m = k + 1; m < S.k_end; ++m) st.q_escaped += (uint64_t)std::llrint(db.dE[m] * 16777216.0f);
             if (end_state) { for (int a = 0; a < 3; ++a) { end_state[a] = FMA(t_cur, g[a], p[a]); end_state[3 + a] = g[a]; } }
+            end_history();
             return;
         }
         for (int a = 0; a < 3; ++a) p[a] = FMA(t_end, g[a], p[a]);
     }
     st.stopped++;
+    end_history();
     if (end_state) { for (int a = 0; a < 3; ++a) { end_state[a] = p[a]; end_state[3 + a] = g[a]; } }
 }
 
@@ -375,7 +405,7 @@ template <class T>
 int run_T(const int16_t *hu, int nx, int ny, int nz, float sx, float sy, float sz,
           const Knot *table, int n_knots, const TrackDB *db, const Beamlet *bl, uint32_t n_bl,
           uint64_t first, uint64_t n, uint64_t stride, uint64_t seed, uint32_t flags,
-          uint64_t *grid, Stats *stats, Trace *tr, T *end_state)
+          uint64_t *grid, Stats *stats, Trace *tr, T *end_state, Squares *sq = nullptr)
 {
     Geometry *G = new Geometry;
     fill_geometry(*G, hu, nx, ny, nz, sx, sy, sz, table, n_knots);
@@ -388,7 +418,7 @@ int run_T(const int16_t *hu, int nx, int ny, int nz, float sx, float sy, float s
         if (rc < 0) break;
         st.protons++;
         if (S.missed) { st.missed++; continue; }
-        transport<T>(*G, *db, S, grid, st, tr, end_state ? end_state + 6 * m : nullptr);
+        transport<T>(*G, *db, S, grid, st, tr, end_state ? end_state + 6 * m : nullptr, sq);
     }
     delete G;
     if (stats) {
@@ -448,6 +478,17 @@ int oracle_run(const int16_t *hu, int nx, int ny, int nz, float sx, float sy, fl
 {
     return run_T<float>(hu, nx, ny, nz, sx, sy, sz, table, n_knots, db, bl, n_bl, first, n, stride, seed, flags,
                         grid, stats, nullptr, nullptr);
+}
+
+/* oracle_run plus the sum-of-squares tallies of R10 (either may be null); all three grids are ADDED to. */
+int oracle_run_sq(const int16_t *hu, int nx, int ny, int nz, float sx, float sy, float sz,
+                  const Knot *table, int n_knots, const TrackDB *db, const Beamlet *bl, uint32_t n_bl,
+                  uint64_t first, uint64_t n, uint64_t stride, uint64_t seed, uint32_t flags,
+                  uint64_t *grid, uint64_t *sq_by_visit, uint64_t *sq_by_history, Stats *stats)
+{
+    Squares sq; sq.by_visit = sq_by_visit; sq.by_history = sq_by_history;
+    return run_T<float>(hu, nx, ny, nz, sx, sy, sz, table, n_knots, db, bl, n_bl, first, n, stride, seed, flags,
+                        grid, stats, nullptr, nullptr, &sq);
 }
 
 /* Same rules evaluated in f64 (error bounding; brute-force and Siddon comparisons). */
