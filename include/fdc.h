@@ -86,7 +86,8 @@ enum {
     FDC_RANDOM_AZIMUTH = 1u,   /* rotate each re-used track by a random azimuth about the beam (R5) */
     FDC_DOSE_TO_HOST   = 2u,   /* dose_gy is a host pointer (else device) */
     FDC_NO_SORT        = 4u,   /* debug: do not group protons by track (same result, slower) */
-    FDC_NO_AGGREGATE   = 8u    /* debug: one atomic per share, no warp aggregation (same result) */
+    FDC_NO_AGGREGATE   = 8u,   /* debug: one atomic per share, no per-voxel merging (same result) */
+    FDC_TALLY_SQUARES  = 16u   /* also tally the sum of squares (second grid; R10) */
 };
 
 /*
@@ -127,6 +128,41 @@ int fdc_get_edep_fixed(fdc_ctx *ctx, uint64_t *grid_out, int is_device_ptr);
 /* Overwrite the raw fixed-point grid, e.g. with the sum over GPUs after an integer all-reduce (the
  * paper's "absorbed dose from both threads was combined"); counters are unchanged. */
 int fdc_set_edep_fixed(fdc_ctx *ctx, const uint64_t *grid_in, int is_device_ptr);
+
+/*
+ * Sum-of-squares tally ("a second tallying array ... the sum of the squares of the
+ * deposited energy", needed by eq. (2)).  fdc_run with FDC_TALLY_SQUARES adds, for every stay of
+ * a proton in a voxel (from entering it to crossing out of it, or to the end of the track), the
+ * square of e' = min((energy left there) >> 8, 2^32 - 1) to a second nx*ny*nz u64 grid (quanta of
+ * 2^-32 MeV^2; R10).  The grid is created zeroed by the first such run and zeroed by
+ * fdc_reset.  Not combinable with FDC_NO_AGGREGATE (FDC_EINVAL).  get: FDC_EINVAL before the first
+ * such run; set (multi-GPU all-reduce) creates the grid if needed.
+ */
+int fdc_get_sq_fixed(fdc_ctx *ctx, uint64_t *grid_out, int is_device_ptr);
+int fdc_set_sq_fixed(fdc_ctx *ctx, const uint64_t *grid_in, int is_device_ptr);
+
+/*
+ * History-by-history statistical uncertainty, eq. (2) (L86; sums over all N primaries),
+ * from the energy grid S1 and the squares grid S2 as they stand, per voxel in f64:
+ *   m = S1*2^-24/N,  m2 = S2*2^-32/N,  sigma = sqrt(max(0, (m2 - m*m)/(N - 1))),  rel = sigma/m (0 if m = 0).
+ * rel_sigma (may be NULL): nx*ny*nz floats, host or device per rel_is_device_ptr.  *mean_rel: the
+ * paper's "mean dose uncertainty" (L92): the average of rel over the voxels whose dose m/rho
+ * exceeds half the maximum dose; *n_voxels_averaged: how many.  Synchronises.  FDC_EINVAL if
+ * n_histories < 2 or no squares grid exists.
+ */
+int fdc_uncertainty_history(fdc_ctx *ctx, uint64_t n_histories, float *rel_sigma, int rel_is_device_ptr,
+                            double *mean_rel, uint64_t *n_voxels_averaged);
+
+/*
+ * Batch-method uncertainty, eq. (1) (L82): batch_grids is a HOST array of n_batches
+ * DEVICE pointers to u64 energy grids (nx*ny*nz, as returned by fdc_get_edep_fixed with a device
+ * pointer), each from an independent run of histories_per_batch histories.  Per voxel in f64:
+ *   mean = (sum_b D_b)/n,  sigma = sqrt(sum_b (D_b - mean)^2 / (n (n - 1))),  rel = sigma/mean,
+ * D_b = grid_b*2^-24 MeV, the sums taken in batch order.  Outputs as fdc_uncertainty_history (the dose for the
+ * half-maximum selection is mean/rho).  2 <= n_batches <= 64.
+ */
+int fdc_uncertainty_batch(fdc_ctx *ctx, const uint64_t *const *batch_grids, int n_batches, uint64_t histories_per_batch,
+                          float *rel_sigma, int rel_is_device_ptr, double *mean_rel, uint64_t *n_voxels_averaged);
 
 /* Counters accumulated since creation / the last fdc_reset (host struct; synchronises). */
 int fdc_get_stats(fdc_ctx *ctx, fdc_stats *out);

@@ -19,11 +19,13 @@ FDC_RANDOM_AZIMUTH = 1
 FDC_DOSE_TO_HOST = 2
 FDC_NO_SORT = 4
 FDC_NO_AGGREGATE = 8
+FDC_TALLY_SQUARES = 16
 
 FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = ["fdc_create", "fdc_load_tracks", "fdc_run", "fdc_get_edep_fixed", "fdc_set_edep_fixed", "fdc_get_stats", "fdc_reset",
-           "fdc_destroy", "fdc_strerror", "fdc_last_error", "fdc_last_timing", "fdc_peak_red_u64"]
+           "fdc_destroy", "fdc_strerror", "fdc_last_error", "fdc_last_timing", "fdc_peak_red_u64",
+           "fdc_get_sq_fixed", "fdc_set_sq_fixed", "fdc_uncertainty_history", "fdc_uncertainty_batch"]
 
 BEAMLET_DTYPE = np.dtype([("origin", "<f4", 3), ("e1", "<f4", 3), ("e2", "<f4", 3), ("dir", "<f4", 3),
                           ("energy_mev", "<f4"), ("spot_u_mm", "<f4"), ("spot_v_mm", "<f4"),
@@ -83,6 +85,13 @@ def lib():
         L.fdc_last_error.argtypes = [vp]
         L.fdc_last_timing.restype = i32
         L.fdc_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float * 4), ctypes.POINTER(u32)]
+        for f in (L.fdc_get_sq_fixed, L.fdc_set_sq_fixed):
+            f.restype = i32
+            f.argtypes = [vp, vp, i32]
+        L.fdc_uncertainty_history.restype = i32
+        L.fdc_uncertainty_history.argtypes = [vp, u64, vp, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
+        L.fdc_uncertainty_batch.restype = i32
+        L.fdc_uncertainty_batch.argtypes = [vp, vp, i32, u64, vp, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
         L.fdc_peak_red_u64.restype = i32
         L.fdc_peak_red_u64.argtypes = [i32, u64, u64, i32, ctypes.POINTER(ctypes.c_double)]
         _lib = L
@@ -174,6 +183,35 @@ class Fdc:
     def fdc_set_edep_fixed(self, grid):
         """Overwrite the raw grid from a CUDA int64 tensor or a host numpy uint64 array."""
         self._check(self._lib.fdc_set_edep_fixed(self._h, _ptr(grid), 1 if _is_device(grid) else 0))
+
+    def fdc_get_sq_fixed(self, out=None):
+        """Sum-of-squares grid (FDC_TALLY_SQUARES); out as in fdc_get_edep_fixed."""
+        if out is None:
+            out = np.empty(self.shape, dtype=np.uint64)
+        self._check(self._lib.fdc_get_sq_fixed(self._h, _ptr(out), 1 if _is_device(out) else 0))
+        return out
+
+    def fdc_set_sq_fixed(self, grid):
+        self._check(self._lib.fdc_set_sq_fixed(self._h, _ptr(grid), 1 if _is_device(grid) else 0))
+
+    def fdc_uncertainty_history(self, n_histories, rel_sigma=None):
+        """Eq. (2).  rel_sigma: None, a CUDA float32 tensor or a host float32 array [nz,ny,nx] (filled).
+        Returns (mean relative uncertainty over voxels above half the maximum dose, their number)."""
+        m = ctypes.c_double(0.0); c = ctypes.c_uint64(0)
+        self._check(self._lib.fdc_uncertainty_history(self._h, int(n_histories), _ptr(rel_sigma),
+                                                      1 if (rel_sigma is not None and _is_device(rel_sigma)) else 0,
+                                                      ctypes.byref(m), ctypes.byref(c)))
+        return m.value, int(c.value)
+
+    def fdc_uncertainty_batch(self, batch_grids, histories_per_batch, rel_sigma=None):
+        """Eq. (1).  batch_grids: list of CUDA int64 tensors [nz,ny,nx] (one energy grid per batch)."""
+        assert all(_is_device(g) and g.is_contiguous() for g in batch_grids)
+        ptrs = (ctypes.c_void_p * len(batch_grids))(*[g.data_ptr() for g in batch_grids])
+        m = ctypes.c_double(0.0); c = ctypes.c_uint64(0)
+        self._check(self._lib.fdc_uncertainty_batch(self._h, ctypes.cast(ptrs, ctypes.c_void_p), len(batch_grids), int(histories_per_batch),
+                                                    _ptr(rel_sigma), 1 if (rel_sigma is not None and _is_device(rel_sigma)) else 0,
+                                                    ctypes.byref(m), ctypes.byref(c)))
+        return m.value, int(c.value)
 
     def fdc_get_stats(self) -> dict:
         s = _Stats()

@@ -237,3 +237,107 @@ def test_config34_full_db_strided_subset(fdc, cfg, n_sub):
         ctx.fdc_run(w.beamlets, 0, w.n_protons // 2, 1, w.seed)
         assert np.array_equal(ctx.fdc_get_edep_fixed(), g)
     ctx.fdc_destroy()
+
+
+def test_config5_full_db_strided_subset(fdc):
+    """Config 5 (512x512x256 grid, 512 MiB of u64: the L2-spill case; 9720 beamlets; 8e5 tracks in
+    the 40 bins the plan touches): the oracle and the GPU run every K-th proton, word for word; then
+    the GPU runs a 1/16 prefix-strided share of the plan in two chunked calls and is checked by
+    conservation and additivity (the whole plan, 2e8 protons, is bench.py --config 5)."""
+    w = fi.workload(5, lazy_db=True)
+    ctx = make_ctx(fdc, w)
+    n_sub = 50_000
+    K = w.n_protons // n_sub
+    check_against_oracle(fdc, w, ctx, first=K // 3, n=n_sub, stride=K)
+    n16 = w.n_protons // 16
+    ctx.fdc_reset()
+    ctx.fdc_run(w.beamlets, 5, n16, 16, w.seed)
+    g = ctx.fdc_get_edep_fixed(); st = ctx.fdc_get_stats()
+    assert st["protons"] == n16 == st["missed"] + st["escaped"] + st["stopped"]
+    assert st["grid_sum"] + st["q_escaped"] == st["q_replayed"] and st["grid_sum"] == int(g.sum(dtype=np.uint64))
+    ctx.fdc_reset()
+    ctx.fdc_run(w.beamlets, 5 + 16 * (n16 // 2), n16 - n16 // 2, 16, w.seed)
+    ctx.fdc_run(w.beamlets, 5, n16 // 2, 16, w.seed)
+    assert np.array_equal(ctx.fdc_get_edep_fixed(), g)
+    ctx.fdc_destroy()
+
+
+
+# ------------------------------------------------------------------ R10 / R11: squares and uncertainties
+def run_gpu_sq(fdc, ctx, w, first=0, n=None, stride=1, seed=None, flags=1):
+    n = w.n_protons if n is None else n
+    ctx.fdc_reset()
+    ctx.fdc_run(w.beamlets, first, n, stride, w.seed if seed is None else seed, flags=flags | fdc.FDC_TALLY_SQUARES)
+    return ctx.fdc_get_edep_fixed(), ctx.fdc_get_sq_fixed(), ctx.fdc_get_stats()
+
+
+@pytest.mark.parametrize("which", ["wl1_small", "wl2_small", "wl3_small"])
+def test_squares_bit_exact(fdc, which, request):
+    """Energy grid, squares grid (by visit, R10) and counters equal the oracle's, word for word; the
+    energy grid is the one the plain run gives."""
+    import oracle
+    w = request.getfixturevalue(which)
+    ctx = make_ctx(fdc, w)
+    with pytest.raises(fdc.FdcError):
+        ctx.fdc_get_sq_fixed()                                                   # no squares grid yet
+    g, s2, st = run_gpu_sq(fdc, ctx, w)
+    og, osv, _, ost = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, by_history=False)
+    assert np.array_equal(g, og) and np.array_equal(s2, osv)
+    for k in STAT_KEYS:
+        assert st[k] == ost[k], (k, st[k], ost[k])
+    with pytest.raises(fdc.FdcError) as e:
+        ctx.fdc_run(w.beamlets, 0, 10, 1, w.seed, flags=1 | fdc.FDC_TALLY_SQUARES | fdc.FDC_NO_AGGREGATE)
+    assert e.value.code == fdc.FDC_EINVAL
+    # additivity and reset
+    g_a, s_a, _ = run_gpu_sq(fdc, ctx, w, first=0, n=w.n_protons // 3)
+    ctx.fdc_run(w.beamlets, w.n_protons // 3, w.n_protons - w.n_protons // 3, 1, w.seed, flags=1 | fdc.FDC_TALLY_SQUARES)
+    assert np.array_equal(ctx.fdc_get_sq_fixed(), s2) and np.array_equal(ctx.fdc_get_edep_fixed(), g)
+    ctx.fdc_reset()
+    assert not ctx.fdc_get_sq_fixed().any()
+    ctx.fdc_destroy()
+
+
+def test_uncertainty_history_and_batch(fdc):
+    """Eq. (2) and eq. (1) maps (f32 of the f64 formula) equal the oracle's numpy evaluation exactly;
+    the mean-uncertainty figure agrees to 1e-8 (fixed-point sum against numpy's pairwise sum)."""
+    import torch
+    import oracle
+    base = fi.workload(1, n_protons=1, tracks_per_bin=500)
+    N = 4000
+    bl = fi.single_beamlet((64.0, 64.0, 0.0), 100.0, 6.0, N)
+    w = fi.Workload("unc", base.phantom, base.table, base.db, bl, N, 31)
+    rho = oracle.density(w.phantom, w.table)
+    ctx = make_ctx(fdc, w)
+    g, s2, _ = run_gpu_sq(fdc, ctx, w)
+    rel = np.zeros(w.phantom.hu.shape, dtype=np.float32)
+    mean_rel, cnt = ctx.fdc_uncertainty_history(N, rel)
+    m, sg = oracle.sigma_history(g, s2, N)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        orel = np.where(m > 0, sg / m, 0.0)
+    assert np.array_equal(rel, orel.astype(np.float32))
+    oval, ocnt = oracle.mean_uncertainty(m, sg, rho)
+    assert cnt == ocnt and mean_rel == pytest.approx(oval, rel=1e-8)
+    rel_d = torch.zeros(w.phantom.hu.shape, dtype=torch.float32, device="cuda")
+    assert ctx.fdc_uncertainty_history(N, rel_d) == (mean_rel, cnt)
+    assert np.array_equal(rel_d.cpu().numpy(), rel)
+    # batches: six independent seeds
+    grids_d, grids_h = [], []
+    for b in range(6):
+        ctx.fdc_reset()
+        ctx.fdc_run(w.beamlets, 0, N, 1, 1000 + b)
+        gd = torch.zeros(w.phantom.hu.shape, dtype=torch.int64, device="cuda")
+        ctx.fdc_get_edep_fixed(gd)
+        grids_d.append(gd); grids_h.append(gd.cpu().numpy().view(np.uint64))
+    relb = np.zeros(w.phantom.hu.shape, dtype=np.float32)
+    mean_b, cnt_b = ctx.fdc_uncertainty_batch(grids_d, N, relb)
+    mb, sb = oracle.sigma_batch(grids_h)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        orelb = np.where(mb > 0, (sb / N) / (mb / N), 0.0)
+    assert np.array_equal(relb, orelb.astype(np.float32))
+    ovalb, ocntb = oracle.mean_uncertainty(mb / N, sb / N, rho)
+    assert cnt_b == ocntb and mean_b == pytest.approx(ovalb, rel=1e-8)
+    # per history the batch figure refers to 6 N histories: it is about sqrt(6) below the single-run one
+    assert mean_rel / mean_b == pytest.approx(np.sqrt(6.0), rel=0.35)
+    with pytest.raises(fdc.FdcError):
+        ctx.fdc_uncertainty_batch(grids_d[:1], N)
+    ctx.fdc_destroy()
