@@ -260,6 +260,34 @@ def run_fdc(args):
                     "h2d_bytes_per_step": int(hu_h.nbytes + sum(a.nbytes for a in host_arrs) + h2d), "d2h_bytes_per_step": d2h,
                     "note": "fdc_create + fdc_load_tracks from pageable host arrays + fdc_run, every step"}
 
+    # ---- PAPER.md:L116 "storing the error in the tally arrays increased the calculation time by 18 %": the same
+    # step with FDC_TALLY_SQUARES (second u64 grid, one more red per voxel left), then eq. (2) on the device
+    unc = None
+    if world == 1 and rank == 0 and not args.no_squares:
+        sq_ms, nsq = 0.0, min(5, args.steps)
+        for it in range(2 + nsq):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            ctx.fdc_reset()
+            ctx.fdc_run(w.beamlets, first, n_mine, 1, w.seed, flags=flags | fdc.FDC_TALLY_SQUARES, dose_gy=dose_d)
+            e1.record()
+            torch.cuda.synchronize()
+            if it >= 2:
+                sq_ms += e0.elapsed_time(e1)
+        t0 = time.perf_counter()
+        mean_rel, n_avg = ctx.fdc_uncertainty_history(n_mine)
+        unc_ms = (time.perf_counter() - t0) * 1e3
+        base_ms = tot_ms / args.steps
+        unc = {"ms_per_step_with_squares": sq_ms / nsq, "squares_cost": sq_ms / nsq / base_ms - 1.0,
+               "paper_squares_cost": 0.18, "mean_rel_uncertainty_eq2": mean_rel, "voxels_above_half_max_dose": n_avg,
+               "histories": n_mine, "eq2_kernels_ms": unc_ms,
+               "seconds_to_1pct_eq2": (sq_ms / nsq * 1e-3) * (mean_rel / 0.01) ** 2 if mean_rel > 0 else None,
+               "note": "PAPER.md:L116-118 context (GTX 295: +18 %, 1 % in about 2 minutes history-by-history); "
+                       "seconds_to_1pct scales this run's time by (mean_rel / 1 %)^2"}
+        ctx.fdc_reset()
+
     if world > 1:
         tl = torch.tensor([st["proton_steps"], st["deposits"], st["protons"]], dtype=torch.int64, device=dev)
         dist.all_reduce(tl)
@@ -331,7 +359,7 @@ def run_fdc(args):
                "e2e_cold": e2e_cold,
                "gpu_launches": int(sum(k["launches"] for k in ktimes)) + (0 if world == 1 else 0),
                "wall_s_timed_region": wall, "clocks": clk, "roofline": roof, "cpu_baseline": cpu,
-               "stats_last_step": st,
+               "uncertainty": unc, "stats_last_step": st,
                "paper_context": "PAPER.md:L114: 184 525 histories/s on one GTX 295 card (other machine, other workload; not a target)"}
         print(json.dumps(out))
     ctx.fdc_destroy()
@@ -350,6 +378,7 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=1_000_000, help="protons of the strided subset the oracle is timed on")
     ap.add_argument("--ref-sample", type=int, default=100_000, help="--impl reference: protons per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-squares", action="store_true", help="skip the FDC_TALLY_SQUARES / eq. (2) leg")
     ap.add_argument("--no-cold", action="store_true", help="skip the e2e_cold leg (context + database re-created from host memory)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "fdc":

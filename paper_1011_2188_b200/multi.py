@@ -28,3 +28,12 @@ def allreduce_edep(ctx, scratch):
     ctx.fdc_get_edep_fixed(scratch)
     allreduce_sum_int64(scratch)
     ctx.fdc_set_edep_fixed(scratch)
+
+
+def allreduce_squares(ctx, scratch):
+    """Same for the sum-of-squares grid (FDC_TALLY_SQUARES): eq. (2)'s sums run over the histories of
+    all ranks, and both sums are integers, so the N-GPU uncertainty map equals the 1-GPU one."""
+    ctx.fdc_get_sq_fixed(scratch)
+    allreduce_sum_int64(scratch)
+    ctx.fdc_set_sq_fixed(scratch)
+
