@@ -29,13 +29,16 @@ def _worker(rank, world, store, out_dir):
     dist.init_process_group("gloo", init_method="file://" + store, rank=rank, world_size=world)
     w = fi.workload(3, n_protons=2352, tracks_per_bin=20)
     first, n = shard_range(w.n_protons, rank, world)
-    g, st = oracle.run(w.phantom, w.table, w.db, w.beamlets, w.seed, first=first, n=n)
+    g, sq, _, st = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, first=first, n=n, by_history=False)
     t = torch.from_numpy(g.view(np.int64))
     allreduce_sum_int64(t)
+    t2 = torch.from_numpy(sq.view(np.int64))                  # the sum-of-squares grid shards the same way
+    allreduce_sum_int64(t2)
     cnt = torch.tensor([st["protons"], st["deposits"]], dtype=torch.int64)
     dist.all_reduce(cnt)
     if rank == 0:
         np.save(os.path.join(out_dir, "grid.npy"), t.numpy().view(np.uint64))
+        np.save(os.path.join(out_dir, "sq.npy"), t2.numpy().view(np.uint64))
         np.save(os.path.join(out_dir, "cnt.npy"), cnt.numpy())
     dist.barrier()
     dist.destroy_process_group()
@@ -49,8 +52,8 @@ def test_two_ranks_sum_to_the_single_rank_grid():
     with tempfile.TemporaryDirectory() as d:
         store = os.path.join(d, "store")
         mp.spawn(_worker, args=(2, store, d), nprocs=2, join=True)
-        g2 = np.load(os.path.join(d, "grid.npy")); cnt = np.load(os.path.join(d, "cnt.npy"))
+        g2 = np.load(os.path.join(d, "grid.npy")); cnt = np.load(os.path.join(d, "cnt.npy")); sq2 = np.load(os.path.join(d, "sq.npy"))
     w = fi.workload(3, n_protons=2352, tracks_per_bin=20)
-    g1, st = oracle.run(w.phantom, w.table, w.db, w.beamlets, w.seed)
-    assert np.array_equal(g1, g2)
+    g1, sq1, _, st = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, by_history=False)
+    assert np.array_equal(g1, g2) and np.array_equal(sq1, sq2)
     assert int(cnt[0]) == st["protons"] == 2352 and int(cnt[1]) == st["deposits"]
