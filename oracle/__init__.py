@@ -126,6 +126,31 @@ def run(phantom, table, db, beamlets, seed, first=0, n=None, stride=1, flags=FLA
     return (grid, d, es) if (f64 and end_state) else (grid, d)
 
 
+PARTICLE_DTYPE = np.dtype([("pos", "<f4", 3), ("dir", "<f4", 3), ("energy_mev", "<f4"), ("reserved", "<f4")], align=True)
+
+
+def run_phase_space(phantom, table, db, particles, seed, first_id=0, flags=FLAG_RANDOM_AZIMUTH):
+    """R12: the path started from a phase-space array.  Returns (grid, stats)."""
+    ps = np.ascontiguousarray(particles, dtype=PARTICLE_DTYPE)
+    grid = np.zeros(phantom.hu.shape, dtype=np.uint64)
+    st = StatsStruct()
+    a, keep = _common_args(phantom, table, db, np.zeros(0, dtype=ps.dtype))
+    a = a[:-2] + [_p(ps), ctypes.c_uint64(len(ps)), ctypes.c_uint64(first_id), ctypes.c_uint64(seed), ctypes.c_uint32(flags),
+                  _p(grid), ctypes.byref(st)]
+    rc = lib().oracle_run_phase_space(*a)
+    if rc != 0:
+        raise RuntimeError("oracle_run_phase_space failed rc=%d" % rc)
+    d = st.as_dict()
+    d["grid_sum"] = int(grid.sum(dtype=np.uint64))
+    return grid, d
+
+
+def frame_rule(d):
+    d = np.ascontiguousarray(d, dtype=np.float32); e1 = np.zeros(3, np.float32); e2 = np.zeros(3, np.float32)
+    lib().oracle_frame_rule(_p(d), _p(e1), _p(e2))
+    return e1, e2
+
+
 def run_sq(phantom, table, db, beamlets, seed, first=0, n=None, stride=1, flags=FLAG_RANDOM_AZIMUTH, by_history=True):
     """Whole path plus the sum-of-squares tallies (R10).  Returns (grid, sq_by_visit,
     sq_by_history or None, stats): u64 grids [nz,ny,nx]; squares in quanta of 2^-32 MeV^2."""

@@ -149,6 +149,9 @@ int energy_bin(float E0, float e_min, float e_bin)
     return x <= 0.0f ? 0 : (int)std::ceil(x);
 }
 
+template <class T>
+int start_from(const Geometry &G, const TrackDB &db, const Beamlet &B, uint64_t i, uint64_t seed, uint32_t flags, Start<T> &S);
+
 /* R2-R6 for proton i.  Returns <0 on FDC_ERANGE-type failure. */
 template <class T>
 int start_proton(const Geometry &G, const TrackDB &db, const Beamlet *bl, uint32_t n_bl,
@@ -158,8 +161,41 @@ int start_proton(const Geometry &G, const TrackDB &db, const Beamlet *bl, uint32
     uint64_t lo = 0; uint32_t b = 0;
     for (; b < n_bl; ++b) { if (i < lo + bl[b].n_protons) break; lo += bl[b].n_protons; }
     if (b == n_bl) return -1;
-    const Beamlet &B = bl[b];
     S.beamlet = b;
+    return start_from<T>(G, db, bl[b], i, seed, flags, S);
+}
+
+/* R12: a phase-space particle (position, unit direction, energy; "phase-space array") is a
+ * one-proton beamlet with no lateral spread whose transverse frame is fixed by its direction d:
+ * a = the axis with the smallest |d_a| (lowest index on ties), t = e_a - d_a d, e1 = t / |t|, e2 = d x e1. */
+struct Particle { float pos[3], dir[3], energy, reserved; };
+void frame_rule(const float d[3], float e1[3], float e2[3])
+{
+    int a = 0;
+    if (std::fabs(d[1]) < std::fabs(d[a])) a = 1;
+    if (std::fabs(d[2]) < std::fabs(d[a])) a = 2;
+    float t[3];
+    for (int b = 0; b < 3; ++b) t[b] = std::fma(-d[a], d[b], b == a ? 1.0f : 0.0f);
+    const float n2 = std::fma(t[2], t[2], std::fma(t[1], t[1], t[0] * t[0]));
+    const float inv = 1.0f / std::sqrt(n2);
+    for (int b = 0; b < 3; ++b) e1[b] = t[b] * inv;
+    e2[0] = std::fma(d[1], e1[2], -(d[2] * e1[1]));
+    e2[1] = std::fma(d[2], e1[0], -(d[0] * e1[2]));
+    e2[2] = std::fma(d[0], e1[1], -(d[1] * e1[0]));
+}
+Beamlet beamlet_of(const Particle &P)
+{
+    Beamlet B; std::memset(&B, 0, sizeof B);
+    for (int a = 0; a < 3; ++a) { B.origin[a] = P.pos[a]; B.dir[a] = P.dir[a]; }
+    frame_rule(P.dir, B.e1, B.e2);
+    B.energy = P.energy; B.spot_u = 0.0f; B.spot_v = 0.0f; B.sigma = 0.0f; B.n_protons = 1;
+    return B;
+}
+
+/* R4-R6 for proton i (its random-number identity) started from beamlet B */
+template <class T>
+int start_from(const Geometry &G, const TrackDB &db, const Beamlet &B, uint64_t i, uint64_t seed, uint32_t flags, Start<T> &S)
+{
     /* R4 */
     int beta = energy_bin(B.energy, db.e_min, db.e_bin);
     if (beta >= (int)db.n_bins) return -2;
@@ -479,6 +515,36 @@ int oracle_run(const int16_t *hu, int nx, int ny, int nz, float sx, float sy, fl
     return run_T<float>(hu, nx, ny, nz, sx, sy, sz, table, n_knots, db, bl, n_bl, first, n, stride, seed, flags,
                         grid, stats, nullptr, nullptr);
 }
+
+/* R12: the path from a phase-space array: particle m is proton first_id + m (random numbers: track
+ * choice and azimuth only).  ADDS into grid and *stats. */
+int oracle_run_phase_space(const int16_t *hu, int nx, int ny, int nz, float sx, float sy, float sz,
+                           const Knot *table, int n_knots, const TrackDB *db, const Particle *ps, uint64_t n,
+                           uint64_t first_id, uint64_t seed, uint32_t flags, uint64_t *grid, Stats *stats)
+{
+    Geometry *G = new Geometry;
+    fill_geometry(*G, hu, nx, ny, nz, sx, sy, sz, table, n_knots);
+    Stats st; std::memset(&st, 0, sizeof st);
+    int rc = 0;
+    for (uint64_t m = 0; m < n; ++m) {
+        const Beamlet B = beamlet_of(ps[m]);
+        Start<float> S; S.beamlet = 0;
+        rc = start_from<float>(*G, *db, B, first_id + m, seed, flags, S);
+        if (rc < 0) break;
+        st.protons++;
+        if (S.missed) { st.missed++; continue; }
+        transport<float>(*G, *db, S, grid, st, nullptr, nullptr);
+    }
+    delete G;
+    if (stats) {
+        stats->protons += st.protons; stats->proton_steps += st.proton_steps; stats->deposits += st.deposits;
+        stats->missed += st.missed; stats->escaped += st.escaped; stats->stopped += st.stopped;
+        stats->q_replayed += st.q_replayed; stats->q_escaped += st.q_escaped;
+    }
+    return rc;
+}
+
+void oracle_frame_rule(const float d[3], float e1[3], float e2[3]) { frame_rule(d, e1, e2); }
 
 /* oracle_run plus the sum-of-squares tallies of R10 (either may be null); all three grids are ADDED to. */
 int oracle_run_sq(const int16_t *hu, int nx, int ny, int nz, float sx, float sy, float sz,
