@@ -59,6 +59,14 @@ typedef struct {
     uint64_t n_protons;
 } fdc_beamlet;
 
+/* One proton of a phase-space array: where it is, where it goes, its kinetic energy. */
+typedef struct {
+    float pos[3];            /* mm, phantom coordinates (may lie outside the grid: R6 moves it to the entry point) */
+    float dir[3];            /* unit vector within 1e-5 */
+    float energy_mev;        /* > 0; must map to a loaded, non-empty energy bin (R4) */
+    float reserved;          /* ignored */
+} fdc_particle;
+
 typedef struct {
     uint64_t protons;        /* protons executed */
     uint64_t proton_steps;   /* database steps begun */
@@ -121,6 +129,22 @@ int fdc_load_tracks(fdc_ctx *ctx, const fdc_trackdb *db, int arrays_are_device_p
 int fdc_run(fdc_ctx *ctx, const fdc_beamlet *b, uint32_t n_beamlets,
             uint64_t first_proton, uint64_t n_protons, uint64_t proton_stride,
             uint64_t seed, uint32_t flags, float *dose_gy);
+
+/*
+ * The same transport started from a phase-space array instead of a beam plan ("the
+ * phase space ... position, direction and energy of the incident protons"; DESIGN.md
+ * R12).  Particle m (ps[m], host or device per ps_is_device_ptr; a host array is copied) is the
+ * proton with random-number identity first_id + m: it draws its track (R4) and azimuth (R5) from
+ * Philox(seed, first_id + m), has no lateral offset, starts at pos along dir with energy_mev, and
+ * its transverse frame is fixed by dir (a = axis of the smallest |dir_a|, lowest index on ties;
+ * e1 = (unit_a - dir_a dir) normalised; e2 = dir x e1).  It then behaves exactly like a one-proton
+ * beamlet with that frame: ADDS to the grid, same flags, same dose_gy convention as fdc_run.
+ * Energies may differ from particle to particle (each starts at the first step with E <= energy).
+ * Errors: FDC_EINVAL (non-finite field, energy <= 0, |dir| != 1), FDC_ERANGE (energy bin outside the
+ * database or empty); the array is validated on the device before anything is tallied.
+ */
+int fdc_run_phase_space(fdc_ctx *ctx, const fdc_particle *ps, uint64_t n, int ps_is_device_ptr,
+                        uint64_t first_id, uint64_t seed, uint32_t flags, float *dose_gy);
 
 /* Copy out the raw fixed-point grid (nx*ny*nz u64, quanta of 2^-24 MeV). */
 int fdc_get_edep_fixed(fdc_ctx *ctx, uint64_t *grid_out, int is_device_ptr);

@@ -25,11 +25,12 @@ FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH 
 
 EXPORTS = ["fdc_create", "fdc_load_tracks", "fdc_run", "fdc_get_edep_fixed", "fdc_set_edep_fixed", "fdc_get_stats", "fdc_reset",
            "fdc_destroy", "fdc_strerror", "fdc_last_error", "fdc_last_timing", "fdc_peak_red_u64",
-           "fdc_get_sq_fixed", "fdc_set_sq_fixed", "fdc_uncertainty_history", "fdc_uncertainty_batch"]
+           "fdc_get_sq_fixed", "fdc_set_sq_fixed", "fdc_uncertainty_history", "fdc_uncertainty_batch", "fdc_run_phase_space"]
 
 BEAMLET_DTYPE = np.dtype([("origin", "<f4", 3), ("e1", "<f4", 3), ("e2", "<f4", 3), ("dir", "<f4", 3),
                           ("energy_mev", "<f4"), ("spot_u_mm", "<f4"), ("spot_v_mm", "<f4"),
                           ("sigma_mm", "<f4"), ("n_protons", "<u8")], align=True)
+PARTICLE_DTYPE = np.dtype([("pos", "<f4", 3), ("dir", "<f4", 3), ("energy_mev", "<f4"), ("reserved", "<f4")], align=True)
 KNOT_DTYPE = np.dtype([("hu", "<f4"), ("density_g_cc", "<f4"), ("mass_spr", "<f4"), ("mass_scpr", "<f4")], align=True)
 
 
@@ -88,6 +89,8 @@ def lib():
         for f in (L.fdc_get_sq_fixed, L.fdc_set_sq_fixed):
             f.restype = i32
             f.argtypes = [vp, vp, i32]
+        L.fdc_run_phase_space.restype = i32
+        L.fdc_run_phase_space.argtypes = [vp, vp, u64, i32, u64, u64, u32, vp]
         L.fdc_uncertainty_history.restype = i32
         L.fdc_uncertainty_history.argtypes = [vp, u64, vp, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
         L.fdc_uncertainty_batch.restype = i32
@@ -172,6 +175,19 @@ class Fdc:
             flags |= FDC_DOSE_TO_HOST
         self._check(self._lib.fdc_run(self._h, _ptr(bl), len(bl), int(first_proton), int(n_protons), int(proton_stride),
                                       int(seed), flags, _ptr(dose_gy)))
+
+    def fdc_run_phase_space(self, particles, first_id, seed, flags=FDC_RANDOM_AZIMUTH, dose_gy=None):
+        """particles: numpy array of PARTICLE_DTYPE (host, copied) or a CUDA uint8/float32 tensor holding
+        n x 32 bytes in that layout (borrowed for the call)."""
+        if isinstance(particles, np.ndarray):
+            ps = np.ascontiguousarray(particles, dtype=PARTICLE_DTYPE); n = len(ps); dev = 0
+        else:
+            ps = particles; n = particles.numel() * particles.element_size() // PARTICLE_DTYPE.itemsize; dev = 1
+            assert particles.is_cuda and particles.is_contiguous()
+        flags = int(flags) & ~FDC_DOSE_TO_HOST
+        if dose_gy is not None and not _is_device(dose_gy):
+            flags |= FDC_DOSE_TO_HOST
+        self._check(self._lib.fdc_run_phase_space(self._h, _ptr(ps), n, dev, int(first_id), int(seed), flags, _ptr(dose_gy)))
 
     def fdc_get_edep_fixed(self, out=None):
         """Raw grid; out: CUDA int64 tensor, or None -> new host numpy uint64 [nz,ny,nx]."""

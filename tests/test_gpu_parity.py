@@ -341,3 +341,59 @@ def test_uncertainty_history_and_batch(fdc):
     with pytest.raises(fdc.FdcError):
         ctx.fdc_uncertainty_batch(grids_d[:1], N)
     ctx.fdc_destroy()
+
+
+# ------------------------------------------------------------------ R12: phase-space source
+def test_phase_space_bit_exact(fdc):
+    """A divergent beam with an energy spread given as a phase-space array: grid and counters equal the
+    oracle's; host and device arrays, identity offsets, additivity, squares; invalid arrays leave no trace."""
+    import torch
+    import oracle
+    from test_oracle_phase_space import cone, particles
+    w = fi.workload(2, n_protons=10, tracks_per_bin=100, lazy_db=False)
+    ctx = make_ctx(fdc, w)
+    ps = cone(5000, 3)
+    og, ost = oracle.run_phase_space(w.phantom, w.table, w.db, ps, 77, first_id=12345)
+    for dev in (False, True):
+        ctx.fdc_reset()
+        arr = torch.from_numpy(ps.view(np.uint8).copy()).cuda() if dev else ps
+        dose = np.zeros(w.phantom.hu.shape, dtype=np.float32)
+        ctx.fdc_run_phase_space(arr, 12345, 77, dose_gy=dose)
+        g = ctx.fdc_get_edep_fixed(); st = ctx.fdc_get_stats()
+        assert np.array_equal(g, og)
+        for k in STAT_KEYS:
+            assert st[k] == ost[k], (k, st[k], ost[k])
+        assert np.array_equal(dose, oracle.to_gy(og, w.phantom, w.table))
+    ctx.fdc_reset()                                                      # two halves, unsorted and squares variants
+    ctx.fdc_run_phase_space(ps[:2000], 12345, 77, flags=1 | fdc.FDC_NO_SORT)
+    ctx.fdc_run_phase_space(ps[2000:], 12345 + 2000, 77, flags=1 | fdc.FDC_TALLY_SQUARES)
+    assert np.array_equal(ctx.fdc_get_edep_fixed(), og)
+    ctx.fdc_reset()
+    ctx.fdc_run_phase_space(ps[:0], 0, 77)                               # empty array: no-op
+    assert ctx.fdc_get_stats()["protons"] == 0
+    bad = ps.copy(); bad["dir"][7] = (0.0, 0.3, 1.0)
+    with pytest.raises(fdc.FdcError) as e:
+        ctx.fdc_run_phase_space(bad, 0, 77)
+    assert e.value.code == fdc.FDC_EINVAL
+    bad = ps.copy(); bad["energy_mev"][11] = 170.0
+    with pytest.raises(fdc.FdcError) as e:
+        ctx.fdc_run_phase_space(bad, 0, 77)
+    assert e.value.code == fdc.FDC_ERANGE
+    assert not ctx.fdc_get_edep_fixed().any() and ctx.fdc_get_stats()["protons"] == 0
+    ctx.fdc_destroy()
+
+
+def test_phase_space_reproduces_beamlet_plan_on_gpu(fdc, wl2_small):
+    """Start points of the beamlet plan handed back as a phase-space array give the plan's own grid."""
+    import oracle
+    from test_oracle_phase_space import particles
+    w = wl2_small
+    ctx = make_ctx(fdc, w)
+    ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed)
+    g_plan = ctx.fdc_get_edep_fixed()
+    smp = oracle.sample(w.phantom, w.table, w.db, w.beamlets, w.seed, first=0, n=w.n_protons)
+    ps = particles(smp["p"], np.tile(np.float32([0, 0, 1]), (w.n_protons, 1)), 150.0)
+    ctx.fdc_reset()
+    ctx.fdc_run_phase_space(ps, 0, w.seed)
+    assert np.array_equal(ctx.fdc_get_edep_fixed(), g_plan)
+    ctx.fdc_destroy()
