@@ -254,3 +254,43 @@ def to_gy(grid, phantom, table):
     lib().oracle_to_gy(_p(g), _p(hu), ctypes.c_uint64(g.size), *[ctypes.c_float(s) for s in phantom.spacing],
                        _p(t), ctypes.c_int(len(t)), _p(dose))
     return dose
+
+
+# ---------------------------------------------------------------- PAPER.md:L94 gamma index (Low et al. 1998), numpy f64
+def gamma_index(dose_ref, dose_eval, spacing, dose_tol_frac=0.03, dist_tol_mm=3.0, search_mm=None, cutoff_frac=0.0):
+    """Discrete gamma index of dose_eval against dose_ref (both [nz,ny,nx] f32), the definition written out:
+    Gamma(r) = min over voxels r' with |r' - r| <= search_mm (offsets in whole voxels, inside the grid) of
+               sqrt(|r' - r|^2 / dist_tol^2 + (D_eval(r') - D_ref(r))^2 / dD^2),   dD = dose_tol_frac * max(D_ref)
+    (global dose criterion; no interpolation between voxels).  Arithmetic in f64 in this order:
+    d2 = ((ox*sx)^2 + (oy*sy)^2) + (oz*sz)^2;  g2 = (diff*diff) * (1/dD^2) + d2 * (1/dist_tol^2).
+    Returns (gamma f32 map, pass fraction = share of voxels with D_ref > cutoff_frac*max(D_ref) whose
+    gamma <= 1, number of such voxels)."""
+    ref = np.asarray(dose_ref, dtype=np.float32).astype(np.float64)
+    ev = np.asarray(dose_eval, dtype=np.float32).astype(np.float64)
+    sx, sy, sz = (float(np.float32(s)) for s in spacing)
+    search = float(np.float32(dist_tol_mm if search_mm is None else search_mm))
+    dmax = float(ref.max())
+    dD = float(np.float32(dose_tol_frac)) * dmax
+    c_dose = 1.0 / (dD * dD)
+    c_dist = 1.0 / (float(np.float32(dist_tol_mm)) * float(np.float32(dist_tol_mm)))
+    rx, ry, rz = int(np.floor(search / sx)), int(np.floor(search / sy)), int(np.floor(search / sz))
+    nz, ny, nx = ref.shape
+    g2 = np.full(ref.shape, np.inf)
+    for oz in range(-rz, rz + 1):
+        for oy in range(-ry, ry + 1):
+            for ox in range(-rx, rx + 1):
+                d2 = ((ox * sx) * (ox * sx) + (oy * sy) * (oy * sy)) + (oz * sz) * (oz * sz)
+                if d2 > search * search:
+                    continue
+                # destination (reference) slices and source (evaluated, shifted by the offset) slices
+                z0, z1 = max(0, -oz), min(nz, nz - oz); y0, y1 = max(0, -oy), min(ny, ny - oy); x0, x1 = max(0, -ox), min(nx, nx - ox)
+                if z0 >= z1 or y0 >= y1 or x0 >= x1:
+                    continue
+                diff = ev[z0 + oz:z1 + oz, y0 + oy:y1 + oy, x0 + ox:x1 + ox] - ref[z0:z1, y0:y1, x0:x1]
+                cand = (diff * diff) * c_dose + d2 * c_dist
+                sub = g2[z0:z1, y0:y1, x0:x1]
+                np.minimum(sub, cand, out=sub)
+    gamma = np.sqrt(g2).astype(np.float32)
+    sel = ref > float(np.float32(cutoff_frac)) * dmax
+    n = int(sel.sum())
+    return gamma, (float((gamma[sel] <= 1.0).sum()) / n if n else 0.0), n
