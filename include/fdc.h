@@ -188,6 +188,19 @@ int fdc_uncertainty_history(fdc_ctx *ctx, uint64_t n_histories, float *rel_sigma
 int fdc_uncertainty_batch(fdc_ctx *ctx, const uint64_t *const *batch_grids, int n_batches, uint64_t histories_per_batch,
                           float *rel_sigma, int rel_is_device_ptr, double *mean_rel, uint64_t *n_voxels_averaged);
 
+/*
+ * Gamma index (Gamma(3 %, 3 mm), Low et al. 1998) of dose_eval against dose_ref,
+ * both DEVICE arrays of nx*ny*nz floats (>= 0) on the context's grid.  Per reference voxel r:
+ *   Gamma(r) = min over whole-voxel offsets o with |o| <= search_mm and r + o inside the grid of
+ *              sqrt(|o|^2 / dist_tol_mm^2 + (D_eval(r + o) - D_ref(r))^2 / dD^2),  dD = dose_tol_frac * max(D_ref)
+ * (global dose criterion, no interpolation; f64, R13).  gamma_out: DEVICE array of nx*ny*nz
+ * floats or NULL.  *pass_fraction: share of the voxels with D_ref > cutoff_frac * max(D_ref) whose
+ * Gamma <= 1; *n_evaluated: their number.  search_mm may cover at most 5 voxels per axis
+ * (FDC_EINVAL otherwise).  Synchronises.
+ */
+int fdc_gamma_index(fdc_ctx *ctx, const float *dose_ref, const float *dose_eval, float dose_tol_frac, float dist_tol_mm,
+                    float search_mm, float cutoff_frac, float *gamma_out, double *pass_fraction, uint64_t *n_evaluated);
+
 /* Counters accumulated since creation / the last fdc_reset (host struct; synchronises). */
 int fdc_get_stats(fdc_ctx *ctx, fdc_stats *out);
 

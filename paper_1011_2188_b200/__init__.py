@@ -25,7 +25,7 @@ FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH 
 
 EXPORTS = ["fdc_create", "fdc_load_tracks", "fdc_run", "fdc_get_edep_fixed", "fdc_set_edep_fixed", "fdc_get_stats", "fdc_reset",
            "fdc_destroy", "fdc_strerror", "fdc_last_error", "fdc_last_timing", "fdc_peak_red_u64",
-           "fdc_get_sq_fixed", "fdc_set_sq_fixed", "fdc_uncertainty_history", "fdc_uncertainty_batch", "fdc_run_phase_space"]
+           "fdc_get_sq_fixed", "fdc_set_sq_fixed", "fdc_uncertainty_history", "fdc_uncertainty_batch", "fdc_run_phase_space", "fdc_gamma_index"]
 
 BEAMLET_DTYPE = np.dtype([("origin", "<f4", 3), ("e1", "<f4", 3), ("e2", "<f4", 3), ("dir", "<f4", 3),
                           ("energy_mev", "<f4"), ("spot_u_mm", "<f4"), ("spot_v_mm", "<f4"),
@@ -91,6 +91,8 @@ def lib():
             f.argtypes = [vp, vp, i32]
         L.fdc_run_phase_space.restype = i32
         L.fdc_run_phase_space.argtypes = [vp, vp, u64, i32, u64, u64, u32, vp]
+        L.fdc_gamma_index.restype = i32
+        L.fdc_gamma_index.argtypes = [vp, vp, vp, f32, f32, f32, f32, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
         L.fdc_uncertainty_history.restype = i32
         L.fdc_uncertainty_history.argtypes = [vp, u64, vp, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
         L.fdc_uncertainty_batch.restype = i32
@@ -228,6 +230,15 @@ class Fdc:
                                                     _ptr(rel_sigma), 1 if (rel_sigma is not None and _is_device(rel_sigma)) else 0,
                                                     ctypes.byref(m), ctypes.byref(c)))
         return m.value, int(c.value)
+
+    def fdc_gamma_index(self, dose_ref, dose_eval, dose_tol_frac=0.03, dist_tol_mm=3.0, search_mm=None, cutoff_frac=0.0, gamma_out=None):
+        """dose_ref, dose_eval, gamma_out: CUDA float32 tensors [nz,ny,nx].  Returns (pass fraction, voxels evaluated)."""
+        assert _is_device(dose_ref) and _is_device(dose_eval) and (gamma_out is None or _is_device(gamma_out))
+        pf = ctypes.c_double(0.0); c = ctypes.c_uint64(0)
+        self._check(self._lib.fdc_gamma_index(self._h, _ptr(dose_ref), _ptr(dose_eval), float(dose_tol_frac), float(dist_tol_mm),
+                                              float(dist_tol_mm if search_mm is None else search_mm), float(cutoff_frac),
+                                              _ptr(gamma_out), ctypes.byref(pf), ctypes.byref(c)))
+        return pf.value, int(c.value)
 
     def fdc_get_stats(self) -> dict:
         s = _Stats()

@@ -397,3 +397,32 @@ def test_phase_space_reproduces_beamlet_plan_on_gpu(fdc, wl2_small):
     ctx.fdc_run_phase_space(ps, 0, w.seed)
     assert np.array_equal(ctx.fdc_get_edep_fixed(), g_plan)
     ctx.fdc_destroy()
+
+
+# ------------------------------------------------------------------ R13: gamma index
+@pytest.mark.parametrize("which,search", [("wl3_small", 3.0), ("wl2_small", 3.0), ("wl2_small", 4.5)])
+def test_gamma_index_bit_exact(fdc, which, search, request):
+    """Two statistically independent runs of the same plan compared with Gamma(3 %, 3 mm), as the paper
+    compares GFDC with GEANT4: the map (f32 of the f64 formula), the pass fraction and
+    the voxel count equal the oracle's definition."""
+    import torch
+    import oracle
+    w = request.getfixturevalue(which)
+    ctx = make_ctx(fdc, w)
+    doses = []
+    for seed in (w.seed, w.seed + 1000):
+        ctx.fdc_reset()
+        d = torch.zeros(w.phantom.hu.shape, dtype=torch.float32, device="cuda")
+        ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, seed, dose_gy=d)
+        doses.append(d)
+    gm = torch.zeros(w.phantom.hu.shape, dtype=torch.float32, device="cuda")
+    for cutoff in (0.0, 0.1):
+        pf, n = ctx.fdc_gamma_index(doses[0], doses[1], 0.03, 3.0, search, cutoff, gm)
+        og, opf, on = oracle.gamma_index(doses[0].cpu().numpy(), doses[1].cpu().numpy(), w.phantom.spacing, 0.03, 3.0, search, cutoff)
+        assert np.array_equal(gm.cpu().numpy(), og)
+        assert n == on and pf == opf
+    pf_same, _ = ctx.fdc_gamma_index(doses[0], doses[0])
+    assert pf_same == 1.0
+    with pytest.raises(fdc.FdcError):
+        ctx.fdc_gamma_index(doses[0], doses[1], 0.03, 3.0, 100.0)                # window of more than 5 voxels
+    ctx.fdc_destroy()
