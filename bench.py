@@ -330,8 +330,16 @@ def run_fdc(args):
             with open(traffic_file) as f:
                 for line in f.read().splitlines()[1:]:
                     c = line.split(",")
-                    if len(c) >= 2 and c[0].strip() == str(args.config):
+                    if len(c) >= 3 and c[0].strip() == str(args.config):
                         roof["traffic"] = float(c[1])
+                        if args.config != 4:        # config 4's capture is one of two launches per step
+                            # third view: the kernel is bound by instruction issue (4 schedulers x 1 warp
+                            # instruction per clock per SM); instructions from the ncu capture, time and clock live
+                            mhz = (clk or {}).get("sm_mhz") or 1965.0
+                            peak_issue = 148 * 4 * mhz * 1e6
+                            roof["issue"] = {"warp_instructions": float(c[2]), "achieved_ginst_s": float(c[2]) / (tr_ms * 1e-3) / 1e9,
+                                             "peak_ginst_s": peak_issue / 1e9, "frac": float(c[2]) / (tr_ms * 1e-3) / peak_issue,
+                                             "note": "instruction count from profiles/ (ncu smsp__inst_executed.sum), kernel time and SM clock from this run"}
 
         # cpu baseline: the oracle on a bounded strided sample, this box's host cores
         cpu = None
