@@ -70,7 +70,8 @@ typedef struct {
 typedef struct {
     uint64_t protons;        /* protons executed */
     uint64_t proton_steps;   /* database steps begun */
-    uint64_t deposits;       /* non-zero shares added to the grid (atomic operations) */
+    uint64_t deposits;       /* non-zero (step, voxel) shares added to the grid (R8); the kernel merges the shares
+                                one proton leaves in one voxel into one atomic, so it issues fewer atomics */
     uint64_t missed;         /* never entered the grid */
     uint64_t escaped;        /* left the grid before the track ended */
     uint64_t stopped;        /* track ended inside the grid */
@@ -101,9 +102,9 @@ enum {
 /*
  * Create a context on `device` using `cuda_stream` (a cudaStream_t; NULL = default stream).
  * hu: nx*ny*nz int16 Hounsfield units, x fastest ("three dimensional array with a
- * material index for each voxel"); values are clamped to [-1024, 3071].  If hu_is_device_ptr the
- * array is BORROWED for the life of the context (the caller keeps it alive and unchanged); a host
- * array is copied before return.  table: n_knots >= 1 knots, strictly increasing in hu, all of
+ * material index for each voxel"); values are clamped to [-1024, 3071].  The array (host, or device if
+ * hu_is_device_ptr) is read during this call only: the library derives its own material-index grid
+ * from it before returning.  table: n_knots >= 1 knots, strictly increasing in hu, all of
  * density, mass_spr, mass_scpr > 0 (host pointer, copied).  Builds the material LUT (R1) and a
  * zeroed u64 energy grid (quantum 2^-24 MeV).
  */

@@ -130,7 +130,7 @@ class Fdc:
     """One fdc_ctx.  Methods mirror the C-ABI one to one."""
 
     def __init__(self, hu, spacing, table, device: int = 0, stream=None):
-        """fdc_create.  hu: int16 [nz,ny,nx] numpy array (copied) or CUDA torch tensor (borrowed)."""
+        """fdc_create.  hu: int16 [nz,ny,nx] numpy array (copied) or CUDA torch tensor (read during the call)."""
         import torch
         self._lib = lib()
         self._h = ctypes.c_void_p(None)
