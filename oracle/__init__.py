@@ -17,6 +17,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 _lib = None
 
 FLAG_RANDOM_AZIMUTH = 1
+FLAG_REALIGN_START = 32
 
 
 class TrackDBStruct(ctypes.Structure):

@@ -230,6 +230,40 @@ int start_from(const Geometry &G, const TrackDB &db, const Beamlet &B, uint64_t 
         S.R[ax][1] = (T)std::fma(c, B.e2[ax], (-s) * B.e1[ax]);
         S.R[ax][2] = (T)B.dir[ax];
     }
+    /* R14 (flag 32): re-align the sub-track.  A proton that starts at step k0 > first re-uses a track
+     * that has already been deflected; with the flag, R0 is followed by the minimal rotation taking the
+     * unit direction u of step k0 to the database z axis, so that the first replayed step points along
+     * the beam (R u = dir).  Same closed form as the R7 rotation with w' = (0,0,1).  Nothing is done if
+     * there is no step to replay, step k0 has zero length, or 1 + u_z < 1e-6. */
+    if ((flags & 32u) && S.k0 < S.k_end) {
+        const T d[3] = {(T)db.dx[S.k0], (T)db.dy[S.k0], (T)db.dz[S.k0]};
+        const T l2 = FMA(d[2], d[2], FMA(d[1], d[1], d[0] * d[0]));
+        if (l2 != (T)0) {
+            const T il = (T)1 / std::sqrt(l2);
+            const T uu[3] = {d[0] * il, d[1] * il, d[2] * il};
+            const T wz[3] = {(T)0, (T)0, (T)1};
+            const T cc = dot3(uu, wz);
+            const T den = (T)1 + cc;
+            if (den >= (T)1e-6f) {
+                T vv[3];
+                vv[0] = FMA(uu[1], wz[2], -(uu[2] * wz[1]));
+                vv[1] = FMA(uu[2], wz[0], -(uu[0] * wz[2]));
+                vv[2] = FMA(uu[0], wz[1], -(uu[1] * wz[0]));
+                const T kk = (T)1 / den;
+                const T kv[3] = {kk * vv[0], kk * vv[1], kk * vv[2]};
+                T dQ[3][3];
+                dQ[0][0] = FMA(kv[0], vv[0], cc); dQ[1][1] = FMA(kv[1], vv[1], cc); dQ[2][2] = FMA(kv[2], vv[2], cc);
+                dQ[0][1] = FMA(kv[0], vv[1], -vv[2]); dQ[1][0] = FMA(kv[0], vv[1], vv[2]);
+                dQ[0][2] = FMA(kv[0], vv[2], vv[1]);  dQ[2][0] = FMA(kv[0], vv[2], -vv[1]);
+                dQ[1][2] = FMA(kv[1], vv[2], -vv[0]); dQ[2][1] = FMA(kv[1], vv[2], vv[0]);
+                T Rn[3][3];
+                for (int a2 = 0; a2 < 3; ++a2)
+                    for (int j2 = 0; j2 < 3; ++j2)
+                        Rn[a2][j2] = FMA(S.R[a2][2], dQ[2][j2], FMA(S.R[a2][1], dQ[1][j2], S.R[a2][0] * dQ[0][j2]));
+                for (int a2 = 0; a2 < 3; ++a2) for (int j2 = 0; j2 < 3; ++j2) S.R[a2][j2] = Rn[a2][j2];
+            }
+        }
+    }
     /* R6 (always in f32: it only places the start point) */
     float hi[3]; bool inside = true;
     for (int ax = 0; ax < 3; ++ax) {
