@@ -96,7 +96,9 @@ enum {
     FDC_DOSE_TO_HOST   = 2u,   /* dose_gy is a host pointer (else device) */
     FDC_NO_SORT        = 4u,   /* debug: do not group protons by track (same result, slower) */
     FDC_NO_AGGREGATE   = 8u,   /* debug: one atomic per share, no per-voxel merging (same result) */
-    FDC_TALLY_SQUARES  = 16u   /* also tally the sum of squares (second grid; R10) */
+    FDC_TALLY_SQUARES  = 16u,  /* also tally the sum of squares (second grid; R10) */
+    FDC_REALIGN_START  = 32u   /* rotate a sub-track that starts at a step k0 > first so that step k0 points along
+                                  the beam (R14); off: the track keeps the deflection it had */
 };
 
 /*

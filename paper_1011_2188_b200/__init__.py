@@ -20,6 +20,7 @@ FDC_DOSE_TO_HOST = 2
 FDC_NO_SORT = 4
 FDC_NO_AGGREGATE = 8
 FDC_TALLY_SQUARES = 16
+FDC_REALIGN_START = 32
 
 FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH = 0, -1, -2, -3, -4, -5, -6
 

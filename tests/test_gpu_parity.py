@@ -46,7 +46,7 @@ def check_against_oracle(fdc, w, ctx=None, flags=1, first=0, n=None, stride=1, s
     ctx.fdc_run(w.beamlets, first, n, stride, seed, flags=flags, dose_gy=dose)
     g = ctx.fdc_get_edep_fixed()
     st = ctx.fdc_get_stats()
-    og, ost = oracle.run(w.phantom, w.table, w.db, w.beamlets, seed, first=first, n=n, stride=stride, flags=flags & 1)
+    og, ost = oracle.run(w.phantom, w.table, w.db, w.beamlets, seed, first=first, n=n, stride=stride, flags=flags & 33)
     assert np.array_equal(g, og), "fixed-point grid differs: %d voxels, sum %d vs %d" % (
         int((g != og).sum()), int(g.sum(dtype=np.uint64)), int(og.sum(dtype=np.uint64)))
     for k in STAT_KEYS:
@@ -425,4 +425,34 @@ def test_gamma_index_bit_exact(fdc, which, search, request):
     assert pf_same == 1.0
     with pytest.raises(fdc.FdcError):
         ctx.fdc_gamma_index(doses[0], doses[1], 0.03, 3.0, 100.0)                # window of more than 5 voxels
+    ctx.fdc_destroy()
+
+
+# ------------------------------------------------------------------ R14: re-aligned deep starts
+def test_realign_start_bit_exact(fdc, wl3_small):
+    """FDC_REALIGN_START against the oracle: a single-energy database entered far below its energy
+    (phase-space energies 60-100 MeV into the 100 MeV bin) from outside the grid and obliquely, and a
+    beam plan; with the flag off the same runs give another grid."""
+    import oracle
+    from test_oracle_phase_space import cone
+    base = fi.workload(1, n_protons=1, tracks_per_bin=300)
+    ctx = make_ctx(fdc, base)
+    ps = cone(3000, 8, e_lo=60.0, e_hi=100.0, half_angle=0.15)
+    grids = {}
+    for flags in (1, 1 | fdc.FDC_REALIGN_START, fdc.FDC_REALIGN_START):
+        ctx.fdc_reset()
+        ctx.fdc_run_phase_space(ps, 500, 21, flags=flags)
+        g = ctx.fdc_get_edep_fixed(); st = ctx.fdc_get_stats()
+        og, ost = oracle.run_phase_space(base.phantom, base.table, base.db, ps, 21, first_id=500, flags=flags)
+        assert np.array_equal(g, og)
+        for k in STAT_KEYS:
+            assert st[k] == ost[k], (k, st[k], ost[k])
+        grids[flags] = g
+    assert not np.array_equal(grids[1], grids[1 | fdc.FDC_REALIGN_START])
+    ctx.fdc_destroy()
+    w = wl3_small
+    ctx = make_ctx(fdc, w)
+    ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed, flags=1 | fdc.FDC_REALIGN_START)
+    og, ost = oracle.run(w.phantom, w.table, w.db, w.beamlets, w.seed, flags=1 | oracle.FLAG_REALIGN_START)
+    assert np.array_equal(ctx.fdc_get_edep_fixed(), og) and ctx.fdc_get_stats()["deposits"] == ost["deposits"]
     ctx.fdc_destroy()
