@@ -306,6 +306,9 @@ def run_fdc(args):
         red_l2 = fdc.fdc_peak_red_u64(local, min(n_vox * 8, 64 << 20), 1 << 30, 0)
         red_fp = red_l2 if n_vox * 8 <= (64 << 20) else fdc.fdc_peak_red_u64(local, n_vox * 8, 1 << 28, 0)
         red_peak = max(red_l2, red_fp)
+        # the same microbenchmark with the 32 lanes of a warp in one 32-byte sector group / on one word
+        red_modes = {"lanes_share_4_words": fdc.fdc_peak_red_u64(local, min(n_vox * 8, 64 << 20), 1 << 28, 1) / 1e9,
+                     "lanes_share_1_word": fdc.fdc_peak_red_u64(local, min(n_vox * 8, 64 << 20), 1 << 28, 2) / 1e9}
         t_track = st["proton_steps"] * STEP_RECORD_BYTES / (hbm_gbs * 1e9)
         t_atomic = st["deposits"] / red_peak
         bound_atomic = t_atomic >= t_track
@@ -320,6 +323,7 @@ def run_fdc(args):
                 "hbm": {"achieved_gbs": st["proton_steps"] * STEP_RECORD_BYTES / (tr_ms * 1e-3) / 1e9, "peak_gbs": hbm_gbs, "peak_source": peak_src},
                 "l2_atomic": {"achieved_gred_s": st["deposits"] / (tr_ms * 1e-3) / 1e9, "peak_gred_s": red_peak / 1e9,
                               "peak_at_grid_footprint_gred_s": red_fp / 1e9, "grid_mib": n_vox * 8 >> 20,
+                              "clustered_peaks_gred_s": red_modes,
                               "peak_source": "fdc_peak_red_u64 measured in this run: u64 red, uniform random addresses over min(grid, 64 MiB) "
                                              "(L2-resident); peak_at_grid_footprint is the same over the whole grid"},
                 "algorithmic": {"proton_steps": st["proton_steps"], "deposits": st["deposits"], "bytes_per_step": STEP_RECORD_BYTES,
