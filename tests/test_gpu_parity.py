@@ -456,3 +456,33 @@ def test_realign_start_bit_exact(fdc, wl3_small):
     og, ost = oracle.run(w.phantom, w.table, w.db, w.beamlets, w.seed, flags=1 | oracle.FLAG_REALIGN_START)
     assert np.array_equal(ctx.fdc_get_edep_fixed(), og) and ctx.fdc_get_stats()["deposits"] == ost["deposits"]
     ctx.fdc_destroy()
+
+
+# ------------------------------------------------------------------ whole plans of configs 3-5 against the off-box oracle
+def _digests():
+    import json
+    import os
+    p = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "full_plan_digests.json")
+    return json.load(open(p))
+
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_plan_digest(fdc, cfg):
+    """BASELINE.json configs[2..4] in full (1e7 / 5e7 / 2e8 protons), the launch configuration bench.py
+    times: the u64 grid's sha256, its sum and every counter equal the ORACLE's, computed off the GPU
+    box by tests/golden/make_digests.py (which calls only oracle/) and stored as text."""
+    import hashlib
+    d = _digests().get(str(cfg))
+    if d is None:
+        pytest.skip("no stored oracle digest for config %d" % cfg)
+    w = fi.workload(cfg, lazy_db=True)
+    assert w.n_protons == d["protons"] and w.seed == d["seed"]
+    ctx = make_ctx(fdc, w)
+    ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed)
+    st = ctx.fdc_get_stats()
+    for k, v in d["stats"].items():
+        assert st[k] == v, (k, st[k], v)
+    g = ctx.fdc_get_edep_fixed()
+    assert list(g.shape) == d["grid_shape"]
+    assert hashlib.sha256(np.ascontiguousarray(g).tobytes()).hexdigest() == d["sha256_u64_grid"]
+    ctx.fdc_destroy()
