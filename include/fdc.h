@@ -6,7 +6,8 @@
  *   fdc_create(CT HU grid, voxel spacing, HU -> density / stopping-power / scattering-power table)
  *   fdc_load_tracks(SoA track database binned by incident energy)
  *   fdc_run(beam fields, proton count, seed) -> dose grid
- * What each call computes is defined rule by rule in DESIGN.md §3 (R1-R9); citations below are
+ * plus the paper's uncertainty estimates, phase-space source and gamma index.
+ * What each call computes is defined rule by rule in DESIGN.md §3 (R1-R14); citations below are
  * PAPER.md line numbers.  Every stage runs in CUDA kernels compiled for sm_100a; there is no CPU
  * fallback (FDC_EARCH on any other device).
  *
