@@ -54,11 +54,31 @@ def digest(cfg, threads):
             "source": "oracle.run over the whole plan of fdc_inputs.workload(%d) (DESIGN.md §5; BASELINE.json configs[%d])" % (cfg, cfg - 1)}
 
 
+def digest_squares(cfg, threads):
+    """The sum-of-squares grid (R10, by visit) of the whole plan: sha256 of its u64 bytes and its sum."""
+    w = fi.workload(cfg, lazy_db=True)
+    parts = threads * 4
+    bounds = [w.n_protons * k // parts for k in range(parts + 1)]
+
+    def work(k):
+        g, sq, _, st = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, first=bounds[k], n=bounds[k + 1] - bounds[k], by_history=False)
+        return sq
+
+    total = np.zeros(w.phantom.hu.shape, dtype=np.uint64)
+    with ThreadPoolExecutor(threads) as ex:
+        for sq in ex.map(work, range(parts)):
+            total += sq
+    return {"sha256_u64_squares": hashlib.sha256(np.ascontiguousarray(total).tobytes()).hexdigest(),
+            "squares_sum_mod_2_64": int(total.sum(dtype=np.uint64))}
+
+
 if __name__ == "__main__":
     cfgs = [int(a) for a in sys.argv[1:]] or [3, 4, 5]
     data = json.load(open(OUT)) if os.path.exists(OUT) else {}
     for c in cfgs:
         data[str(c)] = digest(c, threads=os.cpu_count() or 1)
+        if c == 3:                                   # the squares tally at full size on the one-field plan
+            data[str(c)].update(digest_squares(c, threads=os.cpu_count() or 1))
         print(c, data[str(c)]["sha256_u64_grid"], data[str(c)]["oracle_seconds"], "s", flush=True)
         with open(OUT, "w") as f:
             json.dump(data, f, indent=1, sort_keys=True)

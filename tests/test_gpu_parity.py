@@ -485,4 +485,11 @@ def test_full_plan_digest(fdc, cfg):
     g = ctx.fdc_get_edep_fixed()
     assert list(g.shape) == d["grid_shape"]
     assert hashlib.sha256(np.ascontiguousarray(g).tobytes()).hexdigest() == d["sha256_u64_grid"]
+    if "sha256_u64_squares" in d:                      # R10 at full size
+        ctx.fdc_reset()
+        ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed, flags=1 | fdc.FDC_TALLY_SQUARES)
+        sq = ctx.fdc_get_sq_fixed()
+        assert int(sq.sum(dtype=np.uint64)) == d["squares_sum_mod_2_64"]
+        assert hashlib.sha256(np.ascontiguousarray(sq).tobytes()).hexdigest() == d["sha256_u64_squares"]
+        assert np.array_equal(ctx.fdc_get_edep_fixed(), g)
     ctx.fdc_destroy()
