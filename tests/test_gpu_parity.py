@@ -493,3 +493,33 @@ def test_full_plan_digest(fdc, cfg):
         assert hashlib.sha256(np.ascontiguousarray(sq).tobytes()).hexdigest() == d["sha256_u64_squares"]
         assert np.array_equal(ctx.fdc_get_edep_fixed(), g)
     ctx.fdc_destroy()
+
+
+def test_plan_cache_switches_plans(fdc, wl2_small):
+    """fdc_run keeps the last uploaded plan on the device; switching plans, a zero-proton call with another
+    plan, a failed validation and a database reload in between must not leak the cached one."""
+    import oracle
+    w = wl2_small
+    ctx = make_ctx(fdc, w)
+    other = w.beamlets.copy(); other["spot_u_mm"] += 7.0; other["n_protons"] = 50
+    bad = w.beamlets.copy(); bad["dir"] = (0.0, 0.1, 1.0)
+    og_a, _ = oracle.run(w.phantom, w.table, w.db, w.beamlets, w.seed, n=500)
+    og_b, _ = oracle.run(w.phantom, w.table, w.db, other, w.seed)
+
+    def run(bl, n):
+        ctx.fdc_reset(); ctx.fdc_run(bl, 0, n, 1, w.seed); return ctx.fdc_get_edep_fixed()
+
+    assert np.array_equal(run(w.beamlets, 500), og_a)
+    assert np.array_equal(run(w.beamlets, 500), og_a)                      # cached
+    ctx.fdc_run(other, 0, 0, 1, w.seed)                                      # validated, nothing uploaded
+    with pytest.raises(fdc.FdcError):
+        ctx.fdc_run(other, 0, 51, 1, w.seed)                                 # 51 > other's 50 protons
+    assert np.array_equal(run(w.beamlets, 500), og_a)
+    assert np.array_equal(run(other, 50), og_b)
+    with pytest.raises(fdc.FdcError):
+        ctx.fdc_run(bad, 0, 10, 1, w.seed)
+    assert np.array_equal(run(other, 50), og_b)
+    ctx.fdc_load_tracks(*[np.ascontiguousarray(a) for a in (w.db.dx, w.db.dy, w.db.dz, w.db.dE, w.db.E)],
+                        w.db.track_off, w.db.bin_first, w.db.e_min, w.db.e_bin)
+    assert np.array_equal(run(w.beamlets, 500), og_a)
+    ctx.fdc_destroy()
