@@ -523,3 +523,39 @@ def test_plan_cache_switches_plans(fdc, wl2_small):
                         w.db.track_off, w.db.bin_first, w.db.e_min, w.db.e_bin)
     assert np.array_equal(run(w.beamlets, 500), og_a)
     ctx.fdc_destroy()
+
+
+def test_uncertainty_follows_one_over_sqrt_n_at_scale(fdc):
+    """PAPER.md Fig. 5 / L112 on config 3's plan: the mean dose uncertainty of eq. (2) halves when the
+    histories quadruple, and the batch estimate (eq. (1), six seeds) is of the same size as the
+    history-by-history one for the pooled histories."""
+    import torch
+    w = fi.workload(3)
+    ctx = make_ctx(fdc, w)
+    sq = fdc.FDC_TALLY_SQUARES
+    res = {}
+    for n, stride in ((1_000_000, 10), (4_000_000, 2)):
+        ctx.fdc_reset()
+        ctx.fdc_run(w.beamlets, 0, n, stride, w.seed, flags=1 | sq)
+        res[n] = ctx.fdc_uncertainty_history(n)
+    (u1, c1), (u4, c4) = res[1_000_000], res[4_000_000]
+    assert c1 > 1000 and c4 > 1000
+    assert u1 / u4 == pytest.approx(2.0, rel=0.1)
+    grids = []
+    ctx.fdc_reset()
+    for b in range(6):
+        ctx.fdc_reset()
+        ctx.fdc_run(w.beamlets, 0, 1_000_000, 10, 500 + b)
+        g = torch.zeros(w.phantom.hu.shape, dtype=torch.int64, device="cuda")
+        ctx.fdc_get_edep_fixed(g)
+        grids.append(g)
+    ub, cb = ctx.fdc_uncertainty_batch(grids, 1_000_000)
+    # eq. (2) on the pooled 6e6 histories: the sums of the six runs, squares included
+    ctx.fdc_reset()
+    for b in range(6):
+        ctx.fdc_run(w.beamlets, 0, 1_000_000, 10, 500 + b, flags=1 | sq)
+    uh, ch = ctx.fdc_uncertainty_history(6_000_000)
+    print("mean uncertainty: 1e6 %.4f, 4e6 %.4f, ratio %.3f; six batches of 1e6: batch %.4f, history %.4f, batch/history %.3f" %
+          (u1, u4, u1 / u4, ub, uh, ub / uh))
+    assert 0.6 < ub / uh < 1.6
+    ctx.fdc_destroy()
