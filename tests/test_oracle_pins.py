@@ -452,3 +452,27 @@ def test_f32_contract_close_to_f64(wl3_small):
     a, b = g32.astype(np.float64), g64.astype(np.float64)
     assert np.abs(a - b).sum() / b.sum() < 2e-3
     assert abs(a.sum() - b.sum()) / b.sum() < 1e-4
+
+
+# ------------------------------------------------------------------ P1 / P7 on random degenerate worlds
+def test_conservation_and_additivity_on_random_worlds():
+    """Ragged grids, vacuum to metal, zero-length and very long steps, deflections beyond 90 degrees,
+    oblique beamlets that start inside, outside or miss the grid: energy is conserved exactly, every
+    proton ends in exactly one way, two halves add up to the whole, and the squares tallies are ordered."""
+    from random_worlds import random_case
+    rng = np.random.default_rng(7)
+    seen = dict(missed=0, escaped=0, stopped=0)
+    for case in range(60):
+        w = random_case(rng)
+        flags = int(rng.choice([0, 1, 33]))
+        g, sv, sh, st = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, flags=flags)
+        assert st["grid_sum"] + st["q_escaped"] == st["q_replayed"], case
+        assert st["protons"] == w.n_protons == st["missed"] + st["escaped"] + st["stopped"], case
+        assert np.all(sv <= sh), case
+        h = w.n_protons // 2
+        ga, sa = oracle.run(w.phantom, w.table, w.db, w.beamlets, w.seed, first=0, n=h, flags=flags)
+        gb, sb = oracle.run(w.phantom, w.table, w.db, w.beamlets, w.seed, first=h, n=w.n_protons - h, flags=flags)
+        assert np.array_equal(ga + gb, g) and sa["deposits"] + sb["deposits"] == st["deposits"], case
+        for k in seen:
+            seen[k] += st[k]
+    assert all(v > 100 for v in seen.values()), seen
