@@ -171,6 +171,28 @@ def run_sq(phantom, table, db, beamlets, seed, first=0, n=None, stride=1, flags=
     return grid, sqv, sqh, d
 
 
+def run_secondaries(phantom, table, db, sec, beamlets, seed, first=0, n=None, stride=1, flags=FLAG_RANDOM_AZIMUTH, squares=False):
+    """R15: histories with secondaries.  sec = (sec_first[n_tracks+1], sec_track[n_sec], sec_step[n_sec]) uint32.
+    Returns (grid, stats) or (grid, sq_by_visit, sq_by_history, stats) with squares=True."""
+    if n is None:
+        n = int(beamlets["n_protons"].sum()) - first
+    sf, stt, sst = (np.ascontiguousarray(a, dtype=np.uint32) for a in sec)
+    assert len(sf) == db.n_tracks + 1 and len(stt) == len(sst) == int(sf[-1])
+    grid = np.zeros(phantom.hu.shape, dtype=np.uint64)
+    sqv = np.zeros(phantom.hu.shape, dtype=np.uint64) if squares else None
+    sqh = np.zeros(phantom.hu.shape, dtype=np.uint64) if squares else None
+    st = StatsStruct()
+    a, keep = _common_args(phantom, table, db, beamlets)
+    a = a[:-2] + [_p(sf), _p(stt) if len(stt) else None, _p(sst) if len(sst) else None] + a[-2:]
+    a += _range_args(first, n, stride, seed, flags) + [_p(grid), _p(sqv) if squares else None, _p(sqh) if squares else None, ctypes.byref(st)]
+    rc = lib().oracle_run_secondaries(*a)
+    if rc != 0:
+        raise RuntimeError("oracle_run_secondaries failed rc=%d" % rc)
+    d = st.as_dict()
+    d["grid_sum"] = int(grid.sum(dtype=np.uint64))
+    return (grid, sqv, sqh, d) if squares else (grid, d)
+
+
 # ---------------------------------------------------------------- PAPER.md §2.4, eq. (1), (2), mean uncertainty (numpy f64)
 E_QUANTUM = 2.0 ** -24      # MeV per unit of the energy grid
 SQ_QUANTUM = 2.0 ** -32     # MeV^2 per unit of the squares grid

@@ -316,25 +316,45 @@ struct Trace { uint64_t *voxel; uint64_t *share; uint32_t *step; uint64_t cap, n
 struct Squares { uint64_t *by_visit; uint64_t *by_history; };
 uint64_t sq_operand(uint64_t e) { uint64_t x = e >> 8; if (x > 0xffffffffull) x = 0xffffffffull; return x * x; }
 
-/* R7 + R8 for one proton */
+typedef std::vector<std::pair<uint64_t, uint64_t>> History;    /* every (voxel, share) of one history */
+void reduce_history(History &history, Squares *sq)
+{
+    if (!(sq && sq->by_history)) return;
+    std::sort(history.begin(), history.end());
+    for (size_t a = 0; a < history.size();) {
+        size_t b = a; uint64_t e = 0;
+        while (b < history.size() && history[b].first == history[a].first) { e += history[b].second; ++b; }
+        sq->by_history[history[a].first] += sq_operand(e);
+        a = b;
+    }
+}
+
+/* R15: histories with several trajectories ("each history ... the trajectories"; L71 "selecting
+ * the trajectory").  Secondaries of track j are sec.track[sec.first[j] .. sec.first[j+1]) (tracks outside every
+ * energy bin), each starting where its parent stands at the END of the parent's step number sec.step[] (counted
+ * from the parent's first step; ascending within a parent).  A proton that joins the parent at step k0 skips the
+ * secondaries that branched before k0; one that escapes before a branch step never starts that secondary. */
+struct Secondaries { const uint32_t *first, *track, *step; };
+
+/* R7 + R8 for one trajectory.  spawn: receives the start states of the secondaries whose branch step was completed;
+ * secondary: this trajectory is one (its fate is not counted in escaped / stopped); hist: the history's deposit
+ * list shared by its trajectories (the caller reduces it), or null for a local one. */
 template <class T>
 void transport(const Geometry &G, const TrackDB &db, Start<T> &S, uint64_t *grid, Stats &st, Trace *tr,
-               T *end_state /* p[3], g[3] of the last step, may be null */, Squares *sq = nullptr)
+               T *end_state /* p[3], g[3] of the last step, may be null */, Squares *sq = nullptr,
+               const Secondaries *sec = nullptr, std::vector<Start<T>> *spawn = nullptr, bool secondary = false, History *hist = nullptr)
 {
     uint64_t visit_vox = 0, visit_sum = 0;                       /* R10 by_visit */
-    std::vector<std::pair<uint64_t, uint64_t>> history;          /* R10 by_history: every (voxel, share) of this proton */
+    History local_history;
+    History &history = hist ? *hist : local_history;             /* R10 by_history */
     auto end_visit = [&]() { if (sq && sq->by_visit && visit_sum) sq->by_visit[visit_vox] += sq_operand(visit_sum); visit_sum = 0; };
-    auto end_history = [&]() {
-        end_visit();
-        if (!(sq && sq->by_history)) return;
-        std::sort(history.begin(), history.end());
-        for (size_t a = 0; a < history.size();) {
-            size_t b = a; uint64_t e = 0;
-            while (b < history.size() && history[b].first == history[a].first) { e += history[b].second; ++b; }
-            sq->by_history[history[a].first] += sq_operand(e);
-            a = b;
-        }
-    };
+    auto end_history = [&]() { end_visit(); if (!hist) reduce_history(history, sq); };
+    const uint64_t track_first = db.track_off[S.track];
+    uint32_t s_i = 0, s_end = 0;
+    if (sec && spawn) {
+        s_i = sec->first[S.track]; s_end = sec->first[S.track + 1];
+        while (s_i < s_end && (uint64_t)sec->step[s_i] < S.k0 - track_first) ++s_i;        /* branched before the proton joined */
+    }
     const T INF = std::numeric_limits<T>::infinity();
     const T TINY = (T)7.888609052210118e-31;     /* 2^-100 */
     T p[3] = {S.p[0], S.p[1], S.p[2]};
@@ -359,7 +379,15 @@ void transport(const Geometry &G, const TrackDB &db, Start<T> &S, uint64_t *grid
         };
         const T d[3] = {(T)db.dx[k], (T)db.dy[k], (T)db.dz[k]};
         const T l2 = FMA(d[2], d[2], FMA(d[1], d[1], d[0] * d[0]));
-        if (l2 == (T)0) { deposit(vox, Q); continue; }
+        auto branch_after = [&](uint64_t kk) {                    /* R15: the parent stands at the end of step kk */
+            while (s_i < s_end && (uint64_t)sec->step[s_i] == kk - track_first) {
+                Start<T> B; std::memset(&B, 0, sizeof B);
+                B.track = sec->track[s_i]; B.k0 = db.track_off[B.track]; B.k_end = db.track_off[B.track + 1];
+                for (int a = 0; a < 3; ++a) { B.p[a] = p[a]; B.iv[a] = iv[a]; for (int m = 0; m < 3; ++m) B.R[a][m] = R[a][m]; }
+                spawn->push_back(B); ++s_i;
+            }
+        };
+        if (l2 == (T)0) { deposit(vox, Q); branch_after(k); continue; }
         const T l = std::sqrt(l2);
         const T il = (T)1 / l;
         const T u[3] = {d[0] * il, d[1] * il, d[2] * il};
@@ -450,7 +478,7 @@ void transport(const Geometry &G, const TrackDB &db, Start<T> &S, uint64_t *grid
             vox = (uint64_t)iv[0] + (uint64_t)G.n[0] * ((uint64_t)iv[1] + (uint64_t)G.n[1] * (uint64_t)iv[2]);
         }
         if (escaped) {
-            st.escaped++;
+            if (!secondary) st.escaped++;
             st.q_escaped += Q - q_done;
             for (uint64_t m = k + 1; m < S.k_end; ++m) st.q_escaped += (uint64_t)std::llrint(db.dE[m] * 16777216.0f);
             if (end_state) { for (int a = 0; a < 3; ++a) { end_state[a] = FMA(t_cur, g[a], p[a]); end_state[3 + a] = g[a]; } }
@@ -458,8 +486,9 @@ void transport(const Geometry &G, const TrackDB &db, Start<T> &S, uint64_t *grid
             return;
         }
         for (int a = 0; a < 3; ++a) p[a] = FMA(t_end, g[a], p[a]);
+        branch_after(k);
     }
-    st.stopped++;
+    if (!secondary) st.stopped++;
     end_history();
     if (end_state) { for (int a = 0; a < 3; ++a) { end_state[a] = p[a]; end_state[3 + a] = g[a]; } }
 }
@@ -475,7 +504,7 @@ template <class T>
 int run_T(const int16_t *hu, int nx, int ny, int nz, float sx, float sy, float sz,
           const Knot *table, int n_knots, const TrackDB *db, const Beamlet *bl, uint32_t n_bl,
           uint64_t first, uint64_t n, uint64_t stride, uint64_t seed, uint32_t flags,
-          uint64_t *grid, Stats *stats, Trace *tr, T *end_state, Squares *sq = nullptr)
+          uint64_t *grid, Stats *stats, Trace *tr, T *end_state, Squares *sq = nullptr, const Secondaries *sec = nullptr)
 {
     Geometry *G = new Geometry;
     fill_geometry(*G, hu, nx, ny, nz, sx, sy, sz, table, n_knots);
@@ -488,7 +517,11 @@ int run_T(const int16_t *hu, int nx, int ny, int nz, float sx, float sy, float s
         if (rc < 0) break;
         st.protons++;
         if (S.missed) { st.missed++; continue; }
-        transport<T>(*G, *db, S, grid, st, tr, end_state ? end_state + 6 * m : nullptr, sq);
+        if (!sec) { transport<T>(*G, *db, S, grid, st, tr, end_state ? end_state + 6 * m : nullptr, sq); continue; }
+        std::vector<Start<T>> spawn; History hist;                          /* R15 */
+        transport<T>(*G, *db, S, grid, st, tr, nullptr, sq, sec, &spawn, false, &hist);
+        for (size_t b = 0; b < spawn.size(); ++b) transport<T>(*G, *db, spawn[b], grid, st, tr, nullptr, sq, nullptr, nullptr, true, &hist);
+        reduce_history(hist, sq);
     }
     delete G;
     if (stats) {
@@ -589,6 +622,19 @@ int oracle_run_sq(const int16_t *hu, int nx, int ny, int nz, float sx, float sy,
     Squares sq; sq.by_visit = sq_by_visit; sq.by_history = sq_by_history;
     return run_T<float>(hu, nx, ny, nz, sx, sy, sz, table, n_knots, db, bl, n_bl, first, n, stride, seed, flags,
                         grid, stats, nullptr, nullptr, &sq);
+}
+
+/* R15: oracle_run_sq for a database whose histories have secondaries (squares grids may be null). */
+int oracle_run_secondaries(const int16_t *hu, int nx, int ny, int nz, float sx, float sy, float sz,
+                           const Knot *table, int n_knots, const TrackDB *db, const uint32_t *sec_first, const uint32_t *sec_track,
+                           const uint32_t *sec_step, const Beamlet *bl, uint32_t n_bl,
+                           uint64_t first, uint64_t n, uint64_t stride, uint64_t seed, uint32_t flags,
+                           uint64_t *grid, uint64_t *sq_by_visit, uint64_t *sq_by_history, Stats *stats)
+{
+    Squares sq; sq.by_visit = sq_by_visit; sq.by_history = sq_by_history;
+    Secondaries sec; sec.first = sec_first; sec.track = sec_track; sec.step = sec_step;
+    return run_T<float>(hu, nx, ny, nz, sx, sy, sz, table, n_knots, db, bl, n_bl, first, n, stride, seed, flags,
+                        grid, stats, nullptr, nullptr, &sq, &sec);
 }
 
 /* Same rules evaluated in f64 (error bounding; brute-force and Siddon comparisons). */
