@@ -7,7 +7,7 @@
  *   fdc_load_tracks(SoA track database binned by incident energy)
  *   fdc_run(beam fields, proton count, seed) -> dose grid
  * plus the paper's uncertainty estimates, phase-space source and gamma index.
- * What each call computes is defined rule by rule in DESIGN.md §3 (R1-R14); citations below are
+ * What each call computes is defined rule by rule in DESIGN.md §3 (R1-R15); citations below are
  * PAPER.md line numbers.  Every stage runs in CUDA kernels compiled for sm_100a; there is no CPU
  * fallback (FDC_EARCH on any other device).
  *
@@ -37,7 +37,8 @@ typedef struct { float hu, density_g_cc, mass_spr, mass_scpr; } fdc_knot;
  * loss is stored"), SoA, binned by incident energy.  Step k: displacement (dx,dy,dz) mm, energy
  * loss dE MeV, E[k] = kinetic energy at the start of the step.  Track j owns steps
  * [track_off[j], track_off[j+1]); bin b owns tracks [bin_first[b], bin_first[b+1]) and has nominal
- * energy e_min_mev + b*e_bin_mev.  Requirements (else FDC_EINVAL): offsets non-decreasing and
+ * energy e_min_mev + b*e_bin_mev; bin_first[n_bins] <= n_tracks (tracks past the last bin: see
+ * fdc_set_secondaries).  Requirements (else FDC_EINVAL): offsets non-decreasing and
  * consistent with n_steps / n_tracks; within a track E non-increasing; 0 <= dE < 256; step length
  * either 0 or within [1e-12, 1e6] mm; all values finite. */
 typedef struct {
@@ -120,6 +121,22 @@ int fdc_create(fdc_ctx **out, int device, void *cuda_stream,
  * the library derives its own device-resident step store (unit direction, length, fixed-point
  * energy, suffix sums) before returning, so the caller may free its arrays afterwards. */
 int fdc_load_tracks(fdc_ctx *ctx, const fdc_trackdb *db, int arrays_are_device_ptrs);
+
+/*
+ * Histories with several trajectories (a history holds the primary "and all secondary"
+ * trajectories; L71 "selecting the trajectory"; R15).  Tracks past the last
+ * energy bin (ids >= bin_first[n_bins]; fdc_load_tracks accepts them) are never drawn by R4: they can only
+ * be secondaries.  For parent track j, sec_track[sec_first[j] .. sec_first[j+1]) are its secondaries and
+ * sec_step[] the parent's step (counted from the parent's first step, ascending within a parent) at
+ * whose END each one starts, from the parent's position and frame there, replaying all its own steps
+ * under R7/R8.  A proton that joins the parent at a later step skips the earlier branches; a parent
+ * that escapes before a branch step never starts that secondary.  Counters: escaped / stopped count
+ * primaries; steps, deposits, q_replayed, q_escaped include the secondaries.  At most 6 secondaries
+ * per parent; secondaries have none of their own.  Host arrays, copied.  n_sec = 0 removes the table;
+ * fdc_load_tracks removes it too.  FDC_EINVAL on an inconsistent table, FDC_ENOTRACKS before a load.
+ */
+int fdc_set_secondaries(fdc_ctx *ctx, const uint32_t *sec_first /* n_tracks + 1 */, const uint32_t *sec_track,
+                        const uint32_t *sec_step, uint32_t n_sec);
 
 /*
  * Transport protons and ADD their energy deposits to the context's grid.

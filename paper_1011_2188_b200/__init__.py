@@ -26,7 +26,7 @@ FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH 
 
 EXPORTS = ["fdc_create", "fdc_load_tracks", "fdc_run", "fdc_get_edep_fixed", "fdc_set_edep_fixed", "fdc_get_stats", "fdc_reset",
            "fdc_destroy", "fdc_strerror", "fdc_last_error", "fdc_last_timing", "fdc_peak_red_u64",
-           "fdc_get_sq_fixed", "fdc_set_sq_fixed", "fdc_uncertainty_history", "fdc_uncertainty_batch", "fdc_run_phase_space", "fdc_gamma_index"]
+           "fdc_get_sq_fixed", "fdc_set_sq_fixed", "fdc_uncertainty_history", "fdc_uncertainty_batch", "fdc_run_phase_space", "fdc_gamma_index", "fdc_set_secondaries"]
 
 BEAMLET_DTYPE = np.dtype([("origin", "<f4", 3), ("e1", "<f4", 3), ("e2", "<f4", 3), ("dir", "<f4", 3),
                           ("energy_mev", "<f4"), ("spot_u_mm", "<f4"), ("spot_v_mm", "<f4"),
@@ -92,6 +92,8 @@ def lib():
             f.argtypes = [vp, vp, i32]
         L.fdc_run_phase_space.restype = i32
         L.fdc_run_phase_space.argtypes = [vp, vp, u64, i32, u64, u64, u32, vp]
+        L.fdc_set_secondaries.restype = i32
+        L.fdc_set_secondaries.argtypes = [vp, vp, vp, vp, u32]
         L.fdc_gamma_index.restype = i32
         L.fdc_gamma_index.argtypes = [vp, vp, vp, f32, f32, f32, f32, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
         L.fdc_uncertainty_history.restype = i32
@@ -169,6 +171,13 @@ class Fdc:
                       track_off.ctypes.data, len(track_off) - 1, bin_first.ctypes.data, len(bin_first) - 1,
                       float(e_min), float(e_bin))
         self._check(self._lib.fdc_load_tracks(self._h, ctypes.byref(db), 1 if dev else 0))
+
+    def fdc_set_secondaries(self, sec_first, sec_track, sec_step):
+        """R15 secondary table (numpy uint32 arrays); empty sec_track removes it."""
+        sf = np.ascontiguousarray(sec_first, dtype=np.uint32); stt = np.ascontiguousarray(sec_track, dtype=np.uint32)
+        sst = np.ascontiguousarray(sec_step, dtype=np.uint32)
+        assert len(stt) == len(sst)
+        self._check(self._lib.fdc_set_secondaries(self._h, _ptr(sf), _ptr(stt) if len(stt) else None, _ptr(sst) if len(sst) else None, len(stt)))
 
     def fdc_run(self, beamlets, first_proton, n_protons, proton_stride, seed, flags=FDC_RANDOM_AZIMUTH, dose_gy=None):
         """dose_gy: None, a CUDA float32 tensor [nz,ny,nx], or a host numpy/pinned-torch float32 array."""

@@ -593,3 +593,58 @@ def test_random_degenerate_worlds(fdc):
             og, osv, _, _ = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, by_history=False)
             assert np.array_equal(ctx.fdc_get_edep_fixed(), og) and np.array_equal(ctx.fdc_get_sq_fixed(), osv), case
         ctx.fdc_destroy()
+
+
+# ------------------------------------------------------------------ R15: histories with secondaries
+def test_secondaries_bit_exact(fdc):
+    """Hand-made histories and 60 random degenerate worlds with random secondary tables: grid, squares and
+    counters equal the oracle's with every flag; table validation; the table goes away with n_sec = 0."""
+    import oracle
+    from random_worlds import random_case
+    from test_oracle_secondaries import db_with_secondaries, random_secondaries
+    from test_oracle_pins import table_uniform, uniform_phantom
+    sq = fdc.FDC_TALLY_SQUARES
+
+    def gpu_vs_oracle(ctx, w, db, sec, flags):
+        ctx.fdc_reset()
+        ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed, flags=flags)
+        if flags & sq:
+            og, osv, _, ost = oracle.run_secondaries(w.phantom, w.table, db, sec, w.beamlets, w.seed, flags=flags & 33, squares=True)
+            assert np.array_equal(ctx.fdc_get_sq_fixed(), osv)
+        else:
+            og, ost = oracle.run_secondaries(w.phantom, w.table, db, sec, w.beamlets, w.seed, flags=flags & 33)
+        st = ctx.fdc_get_stats()
+        assert np.array_equal(ctx.fdc_get_edep_fixed(), og)
+        for k in STAT_KEYS:
+            assert st[k] == ost[k], (k, st[k], ost[k])
+
+    ph = uniform_phantom(32, 2.0)
+    prim = [[(0, 0, 1.0, 1.0)] * 10, [(0.1, 0, 1.0, 0.8)] * 7]
+    secs = [(0, 2, [(0.6, 0, 0.8, 2.0)] * 2), (0, 6, [(0, 0.6, 0.8, 3.0)]), (0, 6, [(0, -1.0, 0, 0.5)]), (1, 0, [(1.0, 0, 0, 0.25)] * 3)]
+    db, sec = db_with_secondaries(prim, secs)
+    for e0 in (100.0, 97.5, 93.0):
+        w = fi.Workload("sec", ph, table_uniform(1.0), db, fi.single_beamlet((31.0, 33.0, 1.0), e0, 1.5, 400), 400, 5)
+        ctx = make_ctx(fdc, w)
+        ctx.fdc_set_secondaries(*sec)
+        for flags in (1, 0, 1 | sq, 1 | fdc.FDC_NO_SORT, 1 | fdc.FDC_NO_AGGREGATE, 1 | fdc.FDC_REALIGN_START):
+            gpu_vs_oracle(ctx, w, db, sec, flags)
+        ctx.fdc_set_secondaries(np.zeros(db.n_tracks + 1, np.uint32), [], [])          # removed: the plain run again
+        ctx.fdc_reset(); ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed)
+        g0, _ = oracle.run(w.phantom, w.table, db, w.beamlets, w.seed)
+        assert np.array_equal(ctx.fdc_get_edep_fixed(), g0)
+        bad_first = sec[0].copy(); bad_first[-1] += 1
+        for args in ((bad_first, sec[1], sec[2]), (sec[0], np.zeros_like(sec[1]), sec[2]), (sec[0], sec[1], sec[2] + 100)):
+            with pytest.raises(fdc.FdcError) as e:
+                ctx.fdc_set_secondaries(*args)
+            assert e.value.code == fdc.FDC_EINVAL
+        ctx.fdc_destroy()
+    rng = np.random.default_rng(99)
+    for case in range(60):
+        w0 = random_case(rng)
+        db2, sec2 = random_secondaries(rng, w0.db, None)
+        w = fi.Workload("secfuzz", w0.phantom, w0.table, db2, w0.beamlets, w0.n_protons, w0.seed)
+        ctx = make_ctx(fdc, w)
+        if len(sec2[1]):
+            ctx.fdc_set_secondaries(*sec2)
+        gpu_vs_oracle(ctx, w, db2, sec2, int(rng.choice([0, 1, 1 | sq, 1 | fdc.FDC_REALIGN_START, 1 | fdc.FDC_NO_AGGREGATE])))
+        ctx.fdc_destroy()
