@@ -288,6 +288,36 @@ def run_fdc(args):
                        "seconds_to_1pct scales this run's time by (mean_rel / 1 %)^2"}
         ctx.fdc_reset()
 
+    # ---- R15: the same plan with a synthetic secondary table (fdc_inputs.add_secondaries)
+    sec_leg = None
+    if world == 1 and rank == 0 and not args.no_secondaries:
+        import fdc_inputs as fi
+        db2, sec = fi.add_secondaries(w.db, 1000 + args.config)
+        if len(sec[1]):
+            arrs2 = [np.ascontiguousarray(a) for a in (db2.dx, db2.dy, db2.dz, db2.dE, db2.E)]
+            ctx.fdc_load_tracks(*arrs2, db2.track_off, db2.bin_first, db2.e_min, db2.e_bin)
+            ctx.fdc_set_secondaries(*sec)
+            ms2, n2 = 0.0, min(5, args.steps)
+            for it in range(2 + n2):
+                flush.fill_(1)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record()
+                ctx.fdc_reset()
+                ctx.fdc_run(w.beamlets, first, n_mine, 1, w.seed, flags=flags, dose_gy=dose_d)
+                e1.record()
+                torch.cuda.synchronize()
+                if it >= 2:
+                    ms2 += e0.elapsed_time(e1)
+            st2 = ctx.fdc_get_stats()
+            sec_leg = {"ms_per_step": ms2 / n2, "protons_per_sec": n_mine / (ms2 / n2 * 1e-3), "secondary_tracks": int(len(sec[1])),
+                       "proton_steps": st2["proton_steps"], "deposits": st2["deposits"],
+                       "extra_steps_frac": st2["proton_steps"] / st["proton_steps"] - 1.0,
+                       "extra_time_frac": (ms2 / n2) / (tot_ms / args.steps) - 1.0,
+                       "note": "one synthetic secondary per primary track (tail of another track, 10-40 % of the local energy, "
+                               "10-40 degrees off the parent); k_transport<.,.,SEC>"}
+            ctx.fdc_reset()
+
     if world > 1:
         tl = torch.tensor([st["proton_steps"], st["deposits"], st["protons"]], dtype=torch.int64, device=dev)
         dist.all_reduce(tl)
@@ -371,7 +401,7 @@ def run_fdc(args):
                "e2e_cold": e2e_cold,
                "gpu_launches": int(sum(k["launches"] for k in ktimes)) + (0 if world == 1 else 0),
                "wall_s_timed_region": wall, "clocks": clk, "roofline": roof, "cpu_baseline": cpu,
-               "uncertainty": unc, "stats_last_step": st,
+               "uncertainty": unc, "secondaries": sec_leg, "stats_last_step": st,
                "paper_context": "PAPER.md:L114: 184 525 histories/s on one GTX 295 card (other machine, other workload; not a target)"}
         print(json.dumps(out))
     ctx.fdc_destroy()
@@ -390,6 +420,7 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=1_000_000, help="protons of the strided subset the oracle is timed on")
     ap.add_argument("--ref-sample", type=int, default=100_000, help="--impl reference: protons per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondaries", action="store_true", help="skip the leg with a synthetic secondary table (R15)")
     ap.add_argument("--no-squares", action="store_true", help="skip the FDC_TALLY_SQUARES / eq. (2) leg")
     ap.add_argument("--no-cold", action="store_true", help="skip the e2e_cold leg (context + database re-created from host memory)")
     args = ap.parse_args()

@@ -257,3 +257,56 @@ def workload(cfg: int, n_protons: int | None = None, tracks_per_bin: int | None 
         db = make_trackdb(105, 70.0, 1.0, 181, tpb, bins)
         return Workload("config5_thorax512", ph, material_table("config2"), db, bl, n, 5)
     raise ValueError("cfg must be 1..5")
+
+
+# ----------------------------------------------------------------------------- secondaries (R15), synthetic
+def add_secondaries(db: TrackDB, seed: int, fraction: float = 1.0):
+    """A synthetic secondary table for a generated database (stands in for the secondary
+    trajectories of the paper's GEANT4 histories).  Recipe, per primary track j with at least
+    8 steps, with probability `fraction`: one secondary; it branches at the end of step b = floor(u1 (len - 4));
+    it carries E_s = (0.1 + 0.3 u2) E[b]; its steps are the tail of another primary p of the same database,
+    from that track's first step with E <= E_s on, rotated as a whole so that its first step leaves at polar
+    angle 10 + 30 u3 degrees and azimuth 2 pi u4 from the parent's direction of step b.  u1..u4 and p from
+    numpy's PCG64 seeded by `seed`.  Returns (db with the secondary tracks appended past the last bin,
+    (sec_first, sec_track, sec_step)).  Input preparation only: float64 numpy, rounded to float32."""
+    rng = np.random.default_rng(seed)
+    off = db.track_off.astype(np.int64)
+    n_p = db.n_tracks
+    lens = off[1:] - off[:-1]
+    cand = np.nonzero(lens >= 8)[0]
+    cand = cand[rng.random(len(cand)) < fraction]
+    D = np.stack([db.dx, db.dy, db.dz], 1).astype(np.float64)
+    new_steps, new_dE, new_E, new_len, step_of = [], [], [], [], []
+    pool = np.nonzero(lens > 0)[0]
+    for j in cand:
+        u = rng.random(4)
+        b = int(u[0] * (lens[j] - 4))
+        e_s = (0.1 + 0.3 * u[1]) * float(db.E[off[j] + b])
+        p = int(pool[rng.integers(len(pool))])
+        Ep = db.E[off[p]:off[p + 1]]
+        k = int(np.searchsorted(-Ep, -np.float32(e_s), side="left"))          # first step with E <= E_s (E non-increasing)
+        if k >= lens[p]:
+            continue
+        seg = D[off[p] + k:off[p + 1]]
+        a = seg[0] / max(np.linalg.norm(seg[0]), 1e-30)                       # its own first direction
+        d = D[off[j] + b]; d = d / max(np.linalg.norm(d), 1e-30)              # the parent's direction at the branch
+        th, ph = np.deg2rad(10.0 + 30.0 * u[2]), 2.0 * np.pi * u[3]
+        e1 = np.cross(d, [1.0, 0.0, 0.0] if abs(d[0]) < 0.9 else [0.0, 1.0, 0.0]); e1 /= np.linalg.norm(e1); e2 = np.cross(d, e1)
+        t = np.cos(th) * d + np.sin(th) * (np.cos(ph) * e1 + np.sin(ph) * e2)  # where the secondary leaves
+        v = np.cross(a, t); c = float(a @ t)
+        vx = np.array([[0, -v[2], v[1]], [v[2], 0, -v[0]], [-v[1], v[0], 0]])
+        Rm = np.eye(3) + vx + vx @ vx / (1.0 + c) if c > -0.999999 else -np.eye(3)
+        new_steps.append(seg @ Rm.T); new_dE.append(db.dE[off[p] + k:off[p + 1]]); new_E.append(Ep[k:])
+        new_len.append(len(seg)); step_of.append((int(j), b))
+    if not new_len:
+        return db, (np.zeros(n_p + 1, np.uint32), np.zeros(0, np.uint32), np.zeros(0, np.uint32))
+    S = np.concatenate(new_steps).astype(np.float32)
+    db2 = TrackDB(np.concatenate([db.dx, S[:, 0]]), np.concatenate([db.dy, S[:, 1]]), np.concatenate([db.dz, S[:, 2]]),
+                  np.concatenate([db.dE] + new_dE).astype(np.float32), np.concatenate([db.E] + new_E).astype(np.float32),
+                  np.concatenate([db.track_off, db.track_off[-1] + np.cumsum(new_len).astype(np.uint64)]).astype(np.uint64),
+                  db.bin_first.copy(), db.e_min, db.e_bin)
+    first = np.zeros(db2.n_tracks + 1, dtype=np.int64)
+    for (j, _) in step_of:
+        first[j + 1] += 1
+    first = np.cumsum(first).astype(np.uint32)                                 # candidates ascend in j: the table is already ordered
+    return db2, (first, np.arange(n_p, n_p + len(step_of), dtype=np.uint32), np.array([b for (_, b) in step_of], dtype=np.uint32))

@@ -648,3 +648,24 @@ def test_secondaries_bit_exact(fdc):
             ctx.fdc_set_secondaries(*sec2)
         gpu_vs_oracle(ctx, w, db2, sec2, int(rng.choice([0, 1, 1 | sq, 1 | fdc.FDC_REALIGN_START, 1 | fdc.FDC_NO_AGGREGATE])))
         ctx.fdc_destroy()
+
+
+def test_synthetic_secondaries_on_the_configs(fdc, wl2_small, wl3_small):
+    """fdc_inputs.add_secondaries (the recipe bench.py's secondaries leg uses) on the reduced configs 2 and 3."""
+    import oracle
+    for w0 in (wl2_small, wl3_small):
+        db2, sec = fi.add_secondaries(w0.db, 42)
+        assert len(sec[1]) > 0.5 * w0.db.n_tracks * (w0.db.n_steps > 0)
+        w = fi.Workload("synsec", w0.phantom, w0.table, db2, w0.beamlets, w0.n_protons, w0.seed)
+        ctx = make_ctx(fdc, w)
+        ctx.fdc_set_secondaries(*sec)
+        ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed)
+        og, ost = oracle.run_secondaries(w.phantom, w.table, db2, sec, w.beamlets, w.seed)
+        st = ctx.fdc_get_stats()
+        assert np.array_equal(ctx.fdc_get_edep_fixed(), og)
+        for k in STAT_KEYS:
+            assert st[k] == ost[k], (k, st[k], ost[k])
+        g0, s0 = oracle.run(w0.phantom, w0.table, w0.db, w0.beamlets, w0.seed)
+        assert ost["proton_steps"] > s0["proton_steps"] and ost["q_replayed"] > s0["q_replayed"]
+        ctx.fdc_destroy()
+
