@@ -338,7 +338,10 @@ def run_fdc(args):
         red_peak = max(red_l2, red_fp)
         # the same microbenchmark with the 32 lanes of a warp in one 32-byte sector group / on one word
         red_modes = {"lanes_share_4_words": fdc.fdc_peak_red_u64(local, min(n_vox * 8, 64 << 20), 1 << 28, 1) / 1e9,
-                     "lanes_share_1_word": fdc.fdc_peak_red_u64(local, min(n_vox * 8, 64 << 20), 1 << 28, 2) / 1e9}
+                     "lanes_share_1_word": fdc.fdc_peak_red_u64(local, min(n_vox * 8, 64 << 20), 1 << 28, 2) / 1e9,
+                     # every warp of the GPU on a hot set of a few words (config 1: all protons down one column)
+                     "hot_set_256_words": fdc.fdc_peak_red_u64(local, 256 * 8, 1 << 28, 0) / 1e9,
+                     "hot_set_16_words": fdc.fdc_peak_red_u64(local, 16 * 8, 1 << 26, 0) / 1e9}
         t_track = st["proton_steps"] * STEP_RECORD_BYTES / (hbm_gbs * 1e9)
         t_atomic = st["deposits"] / red_peak
         bound_atomic = t_atomic >= t_track
