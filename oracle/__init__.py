@@ -317,3 +317,42 @@ def gamma_index(dose_ref, dose_eval, spacing, dose_tol_frac=0.03, dist_tol_mm=3.
     sel = ref > float(np.float32(cutoff_frac)) * dmax
     n = int(sel.sum())
     return gamma, (float((gamma[sel] <= 1.0).sum()) / n if n else 0.0), n
+
+
+# ---------------------------------------------------------------- PAPER.md:L104-108 profile comparators, numpy f64
+def profile(values, axis, fixed_a, fixed_b, half_width_a=2, half_width_b=2):
+    """R16 (Fig. 2-3: depth and cross-field profiles, "each profile is calculated along a five voxel
+    thick line").  values: [nz,ny,nx] array (a dose grid, f32; or the u64 energy grid, then the result is in MeV).
+    The line runs along `axis` (0 = x, 1 = y, 2 = z) through the voxel whose indices on the other two axes (a = the
+    lower-numbered one, b = the other) are (fixed_a, fixed_b); it is thickened to the columns with
+    |a - fixed_a| <= half_width_a and |b - fixed_b| <= half_width_b that lie inside the grid, and out[k] is the
+    mean over those columns: summed in f64 with b outer and a inner, then divided by their number.  The energy
+    grid is summed as integers and multiplied once by 2^-24.  Returns float64 [n_axis]."""
+    v = np.asarray(values)
+    nz, ny, nx = v.shape
+    n = (nx, ny, nz)
+    ia, ib = (1 if axis == 0 else 0), (1 if axis == 2 else 2)
+    assert 0 <= fixed_a < n[ia] and 0 <= fixed_b < n[ib]
+    a0, a1 = max(0, fixed_a - half_width_a), min(n[ia] - 1, fixed_a + half_width_a)
+    b0, b1 = max(0, fixed_b - half_width_b), min(n[ib] - 1, fixed_b + half_width_b)
+    is_int = v.dtype.kind in "ui"
+    acc = np.zeros(n[axis], dtype=np.uint64 if is_int else np.float64)
+    for b in range(b0, b1 + 1):
+        for a in range(a0, a1 + 1):
+            idx = [None, None, None]                       # numpy index order is (z, y, x) = axes (2, 1, 0)
+            idx[2 - axis] = slice(None); idx[2 - ia] = a; idx[2 - ib] = b
+            col = v[tuple(idx)]
+            acc = acc + (col.astype(np.uint64) if is_int else col.astype(np.float64))
+    cnt = float((a1 - a0 + 1) * (b1 - b0 + 1))
+    return (acc.astype(np.float64) * E_QUANTUM if is_int else acc) / cnt
+
+
+def rms_diff(dose_ref, dose_eval):
+    """R17 ("the difference between the GFDC- and GEANT4-calculated doses for each voxel in the
+    anatomic phantom divided by the maximum GEANT4 voxel dose has a RMS value of 0.5 %"):
+    sqrt(mean over ALL voxels of ((eval - ref) * (1 / max(ref)))^2), f64.  Returns (rms, max(ref))."""
+    ref = np.asarray(dose_ref, dtype=np.float32).astype(np.float64)
+    ev = np.asarray(dose_eval, dtype=np.float32).astype(np.float64)
+    dmax = float(ref.max())
+    x = (ev - ref) * (1.0 / dmax)
+    return float(np.sqrt(np.sum(x * x) / float(x.size))), dmax
