@@ -3,29 +3,33 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl fdc|reference] [--config C]
 
-One "step" = one pass of the whole hot path over one batch of synthetic input: zero the grid,
-sample + select tracks + group (sort) + transport + deposit + convert to Gy, for every proton of
-the workload.  At N = 1 the workload is BASELINE.json configs[1] (the 128^3 slab phantom, 150 MeV,
-1e6 protons, database of 1e4 tracks per 1 MeV bin over 140-160 MeV), generated from seeds by
-fdc_inputs (synthetic).  Prints ONE JSON line (rank 0).
+One "step" = one pass of the whole hot path over one batch of synthetic input: zero the grid, sample + select
+tracks + group + transport + deposit + convert to Gy, for every proton of the workload.  The workload at N = 1
+is the LARGEST single-GPU configuration, BASELINE.json configs[4] (config 5: 512 x 512 x 256 voxels at 1 mm,
+three fields x 40 layers x 81 spots, 2e8 protons, 2e4 tracks per 1 MeV bin), generated from seeds by fdc_inputs
+(synthetic); `--config C` selects another.  Prints ONE JSON line (rank 0).
 
-`value`   protons/s with every input already resident in HBM (device events, max over ranks).
-`e2e`     the same through the public call with HOST buffers: beam plan H2D and dose grid D2H
-          inside the timed region (the phantom and the track database are resident, loaded once
-          by fdc_create / fdc_load_tracks like weights); `e2e_cold` also re-creates the context
-          and re-loads phantom and database from host memory every step.
-`roofline` the transport+deposit kernel against max(track bytes / HBM peak, deposits / measured
-          u64-red rate) (north_star); see DESIGN.md §8 for the per-unit figures.
+`value`        protons/s with every input already resident in HBM (CUDA events per step, max over ranks).
+`e2e`          the same through the public call with HOST buffers: beam plan H2D (a byte-different, equivalent plan
+               every step, so the library's plan cache cannot skip the upload) and dose grid D2H into pinned host
+               memory inside the timed region; the byte counts are the library's own (fdc_last_call_info).
+               `e2e.cold` also re-creates the context and re-loads phantom and database from host memory each step.
+`roofline`     the transport+deposit kernel against max(track bytes / HBM peak, deposits / measured u64-red rate)
+               (north_star); denominators measured in this run by libfdcpeaks.so, including the red rate over this
+               workload's ACTUAL address multiset (traced by the instrumented kernel, replayed at saturation).
+`per_config`   the other four configs, same process, same L2 flush, same warm-up: ms_per_step, kernel_ms,
+               roofline.frac, deposits ... (N = 1 only).
 `cpu_baseline` the oracle, as it stands, on this box's host cores on a strided proton subset.
 
---impl reference times the oracle (tier framing: the reference arm is the oracle); there is no
-CPU fallback in the product arm: without libfdc.so or a B200 it raises.
+--impl reference times the oracle (tier framing: the reference arm is the oracle); there is no CPU fallback in the
+product arm: without libfdc.so or a B200 it raises.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import subprocess
 import sys
 import threading
 import time
@@ -38,6 +42,7 @@ if ROOT not in sys.path:
 
 L2_FLUSH_BYTES = 512 << 20          # > 126 MB L2
 STEP_RECORD_BYTES = 20              # dx,dy,dz,dE,E float32 per step (north_star (1))
+HEADLINE_CONFIG = 5
 
 
 def _peaks():
@@ -48,12 +53,27 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def _static_counts(cfg):
+    """ncu figures that cannot be measured live (DRAM bytes, warp instructions of one launch): the newest capture
+    of this config's transport kernel, written by hand from profiles/ into profiles/r02_counts.csv with the commit
+    of the kernel it was taken from."""
+    p = os.path.join(ROOT, "profiles", "r02_counts.csv")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        rows = [l.split(",") for l in f.read().splitlines()[1:] if l.strip() and not l.startswith("#")]
+    for c in rows:
+        if c[0].strip() == str(cfg):
+            return {"launch": c[1].strip(), "dram_bytes": float(c[2]), "warp_instructions": float(c[3]), "kernel_ms_under_ncu": float(c[4]),
+                    "source": c[5].strip(), "kernel_commit": c[6].strip()}
+    return None
+
+
 class ClockSampler:
-    """SM clock + throttle reasons sampled through NVML every few ms while the timed region runs
-    (nvidia-smi -lms cannot sample a region that lasts tens of milliseconds)."""
+    """SM clock + throttle reasons sampled through NVML every few ms while the timed region runs."""
     REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
 
-    def __init__(self, index, period_s=0.004):
+    def __init__(self, index, period_s=0.01):
         self.index, self.period, self.samples, self.stop_flag, self.t, self.err = index, period_s, [], False, None, None
 
     def start(self):
@@ -105,11 +125,11 @@ class ClockSampler:
 
 
 def make_workload(cfg, gpus):
-    """configs[cfg-1]; for N > 1 (weak scaling) the plan holds N x the protons and rank r runs the
-    r-th contiguous range of the global proton index space."""
+    """configs[cfg-1]; for N > 1 (weak scaling) the plan holds N x the protons and rank r runs the r-th contiguous
+    range of the global proton index space.  Only the energy bins the plan touches are generated (same tracks)."""
     import fdc_inputs as fi
     base = fi._FULL[cfg]
-    w = fi.workload(cfg, n_protons=base * gpus, lazy_db=(cfg != 2))
+    w = fi.workload(cfg, n_protons=base * gpus, lazy_db=True)
     return w, base
 
 
@@ -146,268 +166,361 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------- product arm
+class Bench:
+    """One workload resident on one GPU: context, database, buffers, the step function and its timers."""
+
+    def __init__(self, cfg, world, rank, local, fdc, torch, dist):
+        from paper_1011_2188_b200 import multi
+        self.fdc, self.torch, self.dist, self.multi = fdc, torch, dist, multi
+        self.cfg, self.world, self.rank, self.local = cfg, world, rank, local
+        self.w, self.per_rank = make_workload(cfg, world)
+        w = self.w
+        self.first, self.n_mine = multi.shard_range(w.n_protons, rank, world)
+        self.dev = torch.device("cuda", local)
+        hu_d = torch.from_numpy(np.ascontiguousarray(w.phantom.hu)).to(self.dev)
+        self.ctx = fdc.Fdc(hu_d, w.phantom.spacing, w.table, device=local)
+        self.host_arrs = [np.ascontiguousarray(a) for a in (w.db.dx, w.db.dy, w.db.dz, w.db.dE, w.db.E)]
+        self.ctx.fdc_load_tracks(*self.host_arrs, w.db.track_off, w.db.bin_first, w.db.e_min, w.db.e_bin)
+        self.dose_d = torch.zeros(w.phantom.hu.shape, dtype=torch.float32, device=self.dev)
+        self.flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=self.dev)
+        self.flags = fdc.FDC_RANDOM_AZIMUTH
+        self.n_vox = int(np.prod(w.phantom.hu.shape))
+
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
+
+    def one_step(self, dose_out, beamlets=None, flags=None):
+        bl = self.w.beamlets if beamlets is None else beamlets
+        self.multi.sharded_step(self.ctx, bl, self.first, self.n_mine, self.w.seed, self.flags if flags is None else flags,
+                                dose_out, self.world)
+
+    def timed(self, n_steps, dose_out, infos=None, flags=None):
+        """n_steps steps, each after an L2 flush, each bracketed by barrier + synchronize; CUDA events; max over ranks."""
+        torch, tot = self.torch, 0.0
+        for _ in range(n_steps):
+            self.flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            self.barrier()
+            e0.record()
+            self.one_step(dose_out, flags=flags)
+            e1.record()
+            self.barrier()
+            ms = e0.elapsed_time(e1)
+            if self.world > 1:
+                t = torch.tensor([ms], device=self.dev); self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX); ms = float(t.item())
+            tot += ms
+            if infos is not None:
+                infos.append(self.ctx.fdc_last_call_info())
+        return tot
+
+    def red_ceilings(self, peaks_cache):
+        """Denominators of the L2-atomic roofline, measured now: u64 red rate over uniformly random
+        addresses in an L2-resident buffer and in a buffer the size of this grid; and over this workload's ACTUAL
+        address multiset: a strided subset of the plan runs through the instrumented kernel (FDC_DIAG_REDS), which
+        records the voxel index of every reduction it sends; libfdcpeaks.so replays that list at saturation, in
+        trace order and shuffled.  Also the count of reductions the kernel really sends for the whole plan."""
+        from paper_1011_2188_b200 import peaks
+        fdc, torch, ctx, w = self.fdc, self.torch, self.ctx, self.w
+        l2_bytes = min(self.n_vox * 8, 64 << 20)
+        key = ("l2", l2_bytes)
+        if key not in peaks_cache:
+            peaks_cache[key] = peaks.red_u64(self.local, l2_bytes, 1 << 30, 0)
+        red_l2 = peaks_cache[key]
+        key = ("fp", self.n_vox * 8)
+        if key not in peaks_cache:
+            peaks_cache[key] = red_l2 if self.n_vox * 8 <= (64 << 20) else peaks.red_u64(self.local, self.n_vox * 8, 1 << 28, 0)
+        red_fp = peaks_cache[key]
+        # whole plan once through the instrumented kernel, no trace buffer: reductions really sent
+        ctx.fdc_reset()
+        ctx.fdc_run(w.beamlets, self.first, self.n_mine, 1, w.seed, flags=self.flags | fdc.FDC_DIAG_REDS)
+        reds_sent = ctx.fdc_last_call_info()["reds_sent"]
+        # strided subset with the trace on
+        n_sub = min(self.n_mine, max(1, int(64e6 * self.n_mine / max(reds_sent, 1))))      # about 64e6 traced addresses
+        K = max(1, self.n_mine // n_sub)
+        cap = int(min(1 << 28, 2 * reds_sent * n_sub // self.n_mine + (1 << 20)))
+        trace = torch.empty(cap, dtype=torch.int32, device=self.dev)
+        ctx.fdc_trace_reds(trace)
+        ctx.fdc_reset()
+        ctx.fdc_run(w.beamlets, self.first, n_sub, K, w.seed, flags=self.flags | fdc.FDC_DIAG_REDS)
+        n_tr = ctx.fdc_last_call_info()["reds_traced"]
+        ctx.fdc_trace_reds(None)
+        ctx.fdc_reset()
+        passes = max(1, int((1 << 29) // max(n_tr, 1)))
+        rep_trace = peaks.red_replay(self.local, trace, n_tr, self.n_vox, passes, False)
+        rep_shuf = peaks.red_replay(self.local, trace, n_tr, self.n_vox, passes, True)
+        del trace
+        return {"peak_gred_s": red_l2 / 1e9, "peak_at_grid_footprint_gred_s": red_fp / 1e9,
+                "peak_actual_multiset_gred_s": rep_shuf / 1e9, "peak_actual_multiset_trace_order_gred_s": rep_trace / 1e9,
+                "multiset_sample": "every %d-th proton (%d protons, %d reductions traced, replayed %d x)" % (K, n_sub, n_tr, passes),
+                "reds_sent_per_step": int(reds_sent), "grid_mib": self.n_vox * 8 >> 20}
+
+    def roofline(self, infos, st, tot_ms, n_steps, ceilings, clk):
+        hbm_gbs, peak_src = _peaks()
+        tr_ms = float(np.mean([k["transport_ms"] for k in infos]))
+        if not tr_ms > 0.0:
+            raise RuntimeError("the library reported no transport time for the timed steps")
+        t_track = st["proton_steps"] * STEP_RECORD_BYTES / (hbm_gbs * 1e9)
+        t_atomic = st["deposits"] / (ceilings["peak_gred_s"] * 1e9)
+        bound_atomic = t_atomic >= t_track
+        n_chunks = max(1, -(-self.n_mine // (1 << 25)))
+        la = dict(ceilings)
+        la.update({"achieved_gred_s": st["deposits"] / (tr_ms * 1e-3) / 1e9,
+                   "sent_gred_s": ceilings["reds_sent_per_step"] / (tr_ms * 1e-3) / 1e9,
+                   "sent_frac_of_peak": ceilings["reds_sent_per_step"] / (tr_ms * 1e-3) / (ceilings["peak_gred_s"] * 1e9),
+                   "sent_frac_of_actual_multiset_peak": ceilings["reds_sent_per_step"] / (tr_ms * 1e-3) / (ceilings["peak_actual_multiset_gred_s"] * 1e9),
+                   "peak_source": "libfdcpeaks.so, measured in this run: u64 red from 2 x 1024 threads per SM; peak = uniform random "
+                                  "addresses over min(grid, 64 MiB) (L2-resident, the denominator of frac: the harder ceiling); "
+                                  "peak_at_grid_footprint = the same over the whole grid; peak_actual_multiset = this workload's traced "
+                                  "voxel indices replayed shuffled (trace_order: as the kernel's warps sent them)"})
+        roof = {"bound": "l2_atomic" if bound_atomic else "hbm",
+                "achieved": la["achieved_gred_s"] if bound_atomic else st["proton_steps"] * STEP_RECORD_BYTES / (tr_ms * 1e-3) / 1e9,
+                "peak": ceilings["peak_gred_s"] if bound_atomic else hbm_gbs,
+                "unit": "Gred/s" if bound_atomic else "GB/s",
+                "frac": max(t_track, t_atomic) / (tr_ms * 1e-3),
+                "traffic": None,
+                "kernel": "k_transport", "kernel_ms": tr_ms, "launches_per_step": n_chunks,
+                "kernel_share_of_step": tr_ms * n_steps / tot_ms,
+                "t_track_ms": t_track * 1e3, "t_atomic_ms": t_atomic * 1e3,
+                "hbm": {"achieved_gbs": st["proton_steps"] * STEP_RECORD_BYTES / (tr_ms * 1e-3) / 1e9, "peak_gbs": hbm_gbs, "peak_source": peak_src},
+                "l2_atomic": la,
+                "algorithmic": {"proton_steps": st["proton_steps"], "deposits": st["deposits"], "bytes_per_step": STEP_RECORD_BYTES,
+                                "note": "achieved counts ALGORITHMIC deposits (non-zero (step, voxel) shares, R8) per step over the "
+                                        "kernel time of the step's launches; the kernel merges the shares one proton leaves in one "
+                                        "voxel into a single reduction, so it SENDS fewer (reds_sent_per_step, sent_gred_s)"}}
+        sc = _static_counts(self.cfg)
+        if sc is not None:
+            mhz = (clk or {}).get("sm_mhz") or 1965.0
+            peak_issue = 148 * 4 * mhz * 1e6
+            roof["traffic"] = sc["dram_bytes"]
+            roof["ncu"] = {"launch": sc["launch"], "dram_bytes_per_launch": sc["dram_bytes"], "warp_instructions_per_launch": sc["warp_instructions"],
+                           "kernel_ms_under_ncu": sc["kernel_ms_under_ncu"],
+                           "issue_frac_under_ncu": sc["warp_instructions"] / (sc["kernel_ms_under_ncu"] * 1e-3) / (148 * 4 * 1965e6),
+                           "source": sc["source"], "kernel_commit": sc["kernel_commit"],
+                           "note": "static: one ncu --set full capture of ONE launch of this config (profiles/), not measured in this run; "
+                                   "issue_frac = warp instructions / (time x 148 SMs x 4 schedulers x 1965 MHz)"}
+            roof["issue_peak_ginst_s_at_sampled_clock"] = peak_issue / 1e9
+        return roof
+
+    def close(self):
+        self.ctx.fdc_destroy()
+        del self.flush, self.dose_d
+        self.torch.cuda.empty_cache()
+
+
+def measure(b, args, peaks_cache, full):
+    """Timed steps + roofline for one resident workload; `full` adds the end-to-end, squares and cpu legs."""
+    fdc, torch, w, ctx = b.fdc, b.torch, b.w, b.ctx
+    warm = max(args.warmup, 3) if not full else args.warmup
+    b.timed(warm, b.dose_d)
+    clocks = ClockSampler(b.local)
+    if b.rank == 0:
+        clocks.start()
+    b.barrier()
+    wall0 = time.perf_counter()
+    infos = []
+    tot_ms = b.timed(args.steps, b.dose_d, infos)
+    b.barrier()
+    wall = time.perf_counter() - wall0
+    clk = clocks.stop() if b.rank == 0 else None
+    st = ctx.fdc_get_stats()                                # counters of the last step (reset each step)
+    res = {"tot_ms": tot_ms, "wall": wall, "clk": clk, "st": st, "infos": infos}
+
+    if b.world > 1:
+        tl = torch.tensor([st["proton_steps"], st["deposits"], st["protons"]], dtype=torch.int64, device=b.dev)
+        b.dist.all_reduce(tl)
+        res["all"] = [int(x) for x in tl.tolist()]
+    else:
+        res["all"] = [st["proton_steps"], st["deposits"], st["protons"]]
+
+    # ---- end to end through the public call with host buffers (every rank; max over ranks)
+    if full:
+        dose_h = torch.empty(w.phantom.hu.shape, dtype=torch.float32).pin_memory()
+        dose_np = dose_h.numpy()
+        # two equivalent plans with different bytes (the second carries one more beamlet of zero protons):
+        # alternating them defeats the library's plan cache, so the plan really crosses the bus every step
+        plan_b = np.concatenate([w.beamlets, w.beamlets[-1:]]); plan_b[-1]["n_protons"] = 0
+        plans = (w.beamlets, plan_b)
+        e2e_ms, h2d, d2h, launches = 0.0, [], [], []
+        for it in range(args.warmup + args.steps):
+            b.flush.fill_(1)
+            b.barrier()
+            t0 = time.perf_counter()
+            b.one_step(dose_np, beamlets=plans[it & 1])     # returns after the D2H copy (synchronises)
+            torch.cuda.synchronize()
+            dt = (time.perf_counter() - t0) * 1e3
+            if b.world > 1:
+                t = torch.tensor([dt], device=b.dev); b.dist.all_reduce(t, op=b.dist.ReduceOp.MAX); dt = float(t.item())
+            if it >= args.warmup:
+                e2e_ms += dt
+                ci = ctx.fdc_last_call_info()
+                h2d.append(ci["h2d_bytes"]); d2h.append(ci["d2h_bytes"]); launches.append(ci["launches"])
+        res["e2e"] = {"value": res["all"][2] * args.steps / (e2e_ms * 1e-3), "unit": "protons/s",
+                      "h2d_bytes_per_step": int(np.mean(h2d)), "d2h_bytes_per_step": int(np.mean(d2h)),
+                      "ms_per_step": e2e_ms / args.steps,
+                      "copies_per_step": "1 H2D plan upload (beamlets + prefix sums) + 1 D2H dose grid, counted by the library "
+                                         "(fdc_last_call_info) in every timed step: min/max h2d %d/%d, d2h %d/%d" % (min(h2d), max(h2d), min(d2h), max(d2h)),
+                      "note": "fdc_reset + fdc_run(host beam plan -> pinned host dose grid), wall clock around the synchronising call; the "
+                              "plan alternates between two byte-different equivalent plans so the plan cache never hits; phantom and "
+                              "track database resident (loaded once, like weights)"}
+        # cold variant: phantom + database from host memory every step (N = 1 only; bounded to 3 steps)
+        if b.world == 1 and not args.no_cold:
+            hu_h = np.ascontiguousarray(w.phantom.hu)
+            cold_ms, ncold = 0.0, min(3, args.steps)
+            for it in range(1 + ncold):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                c2 = fdc.Fdc(hu_h, w.phantom.spacing, w.table, device=b.local)
+                c2.fdc_load_tracks(*b.host_arrs, w.db.track_off, w.db.bin_first, w.db.e_min, w.db.e_bin)
+                c2.fdc_run(w.beamlets, b.first, b.n_mine, 1, w.seed, flags=b.flags, dose_gy=dose_np)
+                torch.cuda.synchronize()
+                if it >= 1:
+                    cold_ms += (time.perf_counter() - t0) * 1e3
+                c2.fdc_destroy()
+            res["e2e"]["cold"] = {"value": b.n_mine * ncold / (cold_ms * 1e-3), "unit": "protons/s", "ms_per_step": cold_ms / ncold, "steps": ncold,
+                                  "h2d_bytes_per_step": int(hu_h.nbytes + sum(a.nbytes for a in b.host_arrs) + res["e2e"]["h2d_bytes_per_step"]),
+                                  "d2h_bytes_per_step": int(dose_np.nbytes),
+                                  "note": "fdc_create + fdc_load_tracks from pageable host arrays + fdc_run, every step"}
+        del dose_h
+
+    # ---- PAPER.md:L116 "storing the error in the tally arrays increased the calculation time by 18 %": the same step
+    # with FDC_TALLY_SQUARES (second u64 grid, one more red per voxel left), then eq. (2) on the device
+    if b.world == 1 and not args.no_squares:
+        nsq = min(5, args.steps)
+        b.timed(2, b.dose_d, flags=b.flags | fdc.FDC_TALLY_SQUARES)
+        sq_ms = b.timed(nsq, b.dose_d, flags=b.flags | fdc.FDC_TALLY_SQUARES)
+        t0 = time.perf_counter()
+        mean_rel, n_avg = ctx.fdc_uncertainty_history(b.n_mine)
+        unc_ms = (time.perf_counter() - t0) * 1e3
+        base_ms = tot_ms / args.steps
+        res["unc"] = {"ms_per_step_with_squares": sq_ms / nsq, "squares_cost": sq_ms / nsq / base_ms - 1.0,
+                      "paper_squares_cost": 0.18, "mean_rel_uncertainty_eq2": mean_rel, "voxels_above_half_max_dose": n_avg,
+                      "histories": b.n_mine, "eq2_kernels_ms": unc_ms,
+                      "seconds_to_1pct_eq2": (sq_ms / nsq * 1e-3) * (mean_rel / 0.01) ** 2 if mean_rel > 0 else None,
+                      "note": "PAPER.md:L116-118 context (GTX 295: +18 %, 1 % in about 2 minutes history-by-history); "
+                              "seconds_to_1pct scales this run's time by (mean_rel / 1 %)^2"}
+        ctx.fdc_reset()
+
+    if b.rank == 0:
+        ceilings = b.red_ceilings(peaks_cache)
+        res["roof"] = b.roofline(infos, st, tot_ms, args.steps, ceilings, clk)
+    return res
+
+
+def secondaries_leg(b, args, base_ms, base_steps):
+    """R15: the same plan with a synthetic secondary table (fdc_inputs.add_secondaries)."""
+    import fdc_inputs as fi
+    w, ctx = b.w, b.ctx
+    db2, sec = fi.add_secondaries(w.db, 1000 + b.cfg)
+    if not len(sec[1]):
+        return None
+    arrs2 = [np.ascontiguousarray(a) for a in (db2.dx, db2.dy, db2.dz, db2.dE, db2.E)]
+    ctx.fdc_load_tracks(*arrs2, db2.track_off, db2.bin_first, db2.e_min, db2.e_bin)
+    ctx.fdc_set_secondaries(*sec)
+    n2 = min(5, args.steps)
+    b.timed(2, b.dose_d)
+    ms2 = b.timed(n2, b.dose_d)
+    st2 = ctx.fdc_get_stats()
+    ctx.fdc_reset()
+    return {"ms_per_step": ms2 / n2, "protons_per_sec": b.n_mine / (ms2 / n2 * 1e-3), "secondary_tracks": int(len(sec[1])),
+            "proton_steps": st2["proton_steps"], "deposits": st2["deposits"],
+            "extra_steps_frac": st2["proton_steps"] / base_steps - 1.0, "extra_time_frac": (ms2 / n2) / base_ms - 1.0,
+            "note": "one synthetic secondary per primary track (tail of another track, 10-40 % of the local energy, 10-40 degrees "
+                    "off the parent); k_transport<.,.,SEC,.>"}
+
+
+def per_config_entry(res, args):
+    roof, st = res["roof"], res["st"]
+    e = {"ms_per_step": res["tot_ms"] / args.steps, "protons_per_sec": res["all"][2] * args.steps / (res["tot_ms"] * 1e-3),
+         "kernel_ms": roof["kernel_ms"], "launches_per_step": roof["launches_per_step"],
+         "roofline": {"bound": roof["bound"], "frac": roof["frac"], "achieved": roof["achieved"], "peak": roof["peak"], "unit": roof["unit"],
+                      "t_track_ms": roof["t_track_ms"], "t_atomic_ms": roof["t_atomic_ms"],
+                      "sent_frac_of_peak": roof["l2_atomic"]["sent_frac_of_peak"],
+                      "peak_at_grid_footprint_gred_s": roof["l2_atomic"]["peak_at_grid_footprint_gred_s"],
+                      "peak_actual_multiset_gred_s": roof["l2_atomic"]["peak_actual_multiset_gred_s"],
+                      "peak_actual_multiset_trace_order_gred_s": roof["l2_atomic"]["peak_actual_multiset_trace_order_gred_s"]},
+         "issue": ({"frac_under_ncu": roof["ncu"]["issue_frac_under_ncu"], "warp_instructions_per_launch": roof["ncu"]["warp_instructions_per_launch"],
+                    "launch": roof["ncu"]["launch"], "source": roof["ncu"]["source"], "kernel_commit": roof["ncu"]["kernel_commit"]}
+                   if "ncu" in roof else None),
+         "protons": st["protons"], "proton_steps": st["proton_steps"], "deposits": st["deposits"],
+         "reds_sent": roof["l2_atomic"]["reds_sent_per_step"], "clocks": res["clk"], "steps": args.steps, "warmup": max(args.warmup, 3)}
+    if "unc" in res:
+        e["squares_cost"] = res["unc"]["squares_cost"]; e["mean_rel_uncertainty_eq2"] = res["unc"]["mean_rel_uncertainty_eq2"]
+    return e
+
+
 def run_fdc(args):
     import torch
     import torch.distributed as dist
     import paper_1011_2188_b200 as fdc
-    from paper_1011_2188_b200 import multi
+    from paper_1011_2188_b200 import peaks
     fdc.lib()                                             # no fallback: raises if the library is missing
+    peaks.lib()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a B200; there is no CPU fallback (use --impl reference for the oracle)")
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise RuntimeError("--gpus %d but WORLD_SIZE=%d: launch with torch.distributed.run --nproc-per-node %d" % (args.gpus, world, args.gpus))
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    w, per_rank = make_workload(args.config, world)
-    first, n_mine = multi.shard_range(w.n_protons, rank, world)
-    dev = torch.device("cuda", local)
+    peaks_cache = {}
 
-    # resident inputs (borrowed device arrays; PyTorch = device memory and streams only)
-    hu_d = torch.from_numpy(np.ascontiguousarray(w.phantom.hu)).to(dev)
-    ctx = fdc.Fdc(hu_d, w.phantom.spacing, w.table, device=local)
-    host_arrs = [np.ascontiguousarray(a) for a in (w.db.dx, w.db.dy, w.db.dz, w.db.dE, w.db.E)]
-    ctx.fdc_load_tracks(*host_arrs, w.db.track_off, w.db.bin_first, w.db.e_min, w.db.e_bin)
-    dose_d = torch.zeros(w.phantom.hu.shape, dtype=torch.float32, device=dev)
-    grid_d = torch.zeros(w.phantom.hu.shape, dtype=torch.int64, device=dev) if world > 1 else None
-    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
-    flags = fdc.FDC_RANDOM_AZIMUTH
+    b = Bench(args.config, world, rank, local, fdc, torch, dist)
+    res = measure(b, args, peaks_cache, full=True)
+    w = b.w
+    tot_ms, st, infos = res["tot_ms"], res["st"], res["infos"]
+    all_steps, all_deps, all_prot = res["all"]
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    def one_step(dose_out):
-        ctx.fdc_reset()
-        if world == 1:
-            ctx.fdc_run(w.beamlets, first, n_mine, 1, w.seed, flags=flags, dose_gy=dose_out)
-        else:
-            ctx.fdc_run(w.beamlets, first, n_mine, 1, w.seed, flags=flags)
-            multi.allreduce_edep(ctx, grid_d)              # the paper's "dose from both threads was combined" (L75)
-            ctx.fdc_run(w.beamlets, 0, 0, 1, w.seed, flags=flags, dose_gy=dose_out)
-
-    def timed(n_steps, dose_out, kernel_times=None):
-        tot = 0.0
-        for _ in range(n_steps):
-            flush.fill_(1)                                  # L2 flush between timed iterations
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            barrier()
-            e0.record()
-            one_step(dose_out)
-            e1.record()
-            barrier()
-            ms = e0.elapsed_time(e1)
-            if world > 1:
-                t = torch.tensor([ms], device=dev); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms = float(t.item())
-            tot += ms
-            if kernel_times is not None:
-                kernel_times.append(ctx.fdc_last_timing())
-        return tot
-
-    timed(args.warmup, dose_d)
-    clocks = ClockSampler(local)
-    if rank == 0:
-        clocks.start()
-    barrier()
-    wall0 = time.perf_counter()
-    ktimes = []
-    tot_ms = timed(args.steps, dose_d, ktimes)
-    barrier()
-    wall = time.perf_counter() - wall0
-    clk = clocks.stop() if rank == 0 else None
-    st = ctx.fdc_get_stats()                                # counters of the last step (reset each step)
-
-    # ---- end to end through the public call with host buffers
-    dose_h = torch.empty(w.phantom.hu.shape, dtype=torch.float32).pin_memory()
-    dose_np = dose_h.numpy()
-
-    def e2e_step():
-        one_step(dose_np)                                   # beam plan H2D + dose D2H inside fdc_run (synchronises)
-
-    e2e_ms = 0.0
-    for it in range(args.warmup + args.steps):
-        flush.fill_(1)
-        barrier()
+    # cpu baseline: the oracle on a bounded strided sample, this box's host cores
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        n_sub = min(args.cpu_sample, w.n_protons)
+        K = max(1, w.n_protons // n_sub)
         t0 = time.perf_counter()
-        e2e_step()
-        torch.cuda.synchronize()
-        dt = (time.perf_counter() - t0) * 1e3
-        if world > 1:
-            t = torch.tensor([dt], device=dev); dist.all_reduce(t, op=dist.ReduceOp.MAX); dt = float(t.item())
-        if it >= args.warmup:
-            e2e_ms += dt
-    h2d = int(w.beamlets.nbytes + 8 * (len(w.beamlets) + 1))
-    d2h = int(dose_np.nbytes)
+        og, ost = oracle.run(w.phantom, w.table, w.db, w.beamlets, w.seed, first=0, n=n_sub, stride=K)
+        dt = time.perf_counter() - t0
+        cpu = {"value": n_sub / dt, "unit": "protons/s", "cores": 1, "kind": "oracle", "host_cores_available": os.cpu_count(),
+               "steps_per_sec": ost["proton_steps"] / dt,
+               "sample": "every %d-th proton of %s (%d protons, %.1f s), single thread" % (K, w.name, n_sub, dt)}
+    config = {"workload": w.name, "protons_per_step": all_prot, "protons_per_gpu": b.per_rank, "grid": list(w.phantom.dims),
+              "db_tracks": w.db.n_tracks, "db_steps": w.db.n_steps, "beamlets": len(w.beamlets),
+              "parallelism": "proton ranges x%d, in-place u64 grid all-reduce (NCCL)" % world if world > 1 else "single GPU",
+              "l2": "flushed between timed steps (512 MiB write)", "timer": "CUDA events per step, max over ranks"}
+    launches = int(sum(k["launches"] for k in infos))
+    b.close()
 
-    # cold variant: phantom + database from host memory every step (N = 1 only; bounded to 3 steps)
-    e2e_cold = None
-    if world == 1 and rank == 0 and not args.no_cold:
-        hu_h = np.ascontiguousarray(w.phantom.hu)
-        cold_ms, ncold = 0.0, min(3, args.steps)
-        for it in range(1 + ncold):
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            c2 = fdc.Fdc(hu_h, w.phantom.spacing, w.table, device=local)
-            c2.fdc_load_tracks(*host_arrs, w.db.track_off, w.db.bin_first, w.db.e_min, w.db.e_bin)
-            c2.fdc_run(w.beamlets, first, n_mine, 1, w.seed, flags=flags, dose_gy=dose_np)
-            torch.cuda.synchronize()
-            if it >= 1:
-                cold_ms += (time.perf_counter() - t0) * 1e3
-            c2.fdc_destroy()
-        e2e_cold = {"value": n_mine * ncold / (cold_ms * 1e-3), "unit": "protons/s",
-                    "h2d_bytes_per_step": int(hu_h.nbytes + sum(a.nbytes for a in host_arrs) + h2d), "d2h_bytes_per_step": d2h,
-                    "note": "fdc_create + fdc_load_tracks from pageable host arrays + fdc_run, every step"}
-
-    # ---- PAPER.md:L116 "storing the error in the tally arrays increased the calculation time by 18 %": the same
-    # step with FDC_TALLY_SQUARES (second u64 grid, one more red per voxel left), then eq. (2) on the device
-    unc = None
-    if world == 1 and rank == 0 and not args.no_squares:
-        sq_ms, nsq = 0.0, min(5, args.steps)
-        for it in range(2 + nsq):
-            flush.fill_(1)
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize()
-            e0.record()
-            ctx.fdc_reset()
-            ctx.fdc_run(w.beamlets, first, n_mine, 1, w.seed, flags=flags | fdc.FDC_TALLY_SQUARES, dose_gy=dose_d)
-            e1.record()
-            torch.cuda.synchronize()
-            if it >= 2:
-                sq_ms += e0.elapsed_time(e1)
-        t0 = time.perf_counter()
-        mean_rel, n_avg = ctx.fdc_uncertainty_history(n_mine)
-        unc_ms = (time.perf_counter() - t0) * 1e3
-        base_ms = tot_ms / args.steps
-        unc = {"ms_per_step_with_squares": sq_ms / nsq, "squares_cost": sq_ms / nsq / base_ms - 1.0,
-               "paper_squares_cost": 0.18, "mean_rel_uncertainty_eq2": mean_rel, "voxels_above_half_max_dose": n_avg,
-               "histories": n_mine, "eq2_kernels_ms": unc_ms,
-               "seconds_to_1pct_eq2": (sq_ms / nsq * 1e-3) * (mean_rel / 0.01) ** 2 if mean_rel > 0 else None,
-               "note": "PAPER.md:L116-118 context (GTX 295: +18 %, 1 % in about 2 minutes history-by-history); "
-                       "seconds_to_1pct scales this run's time by (mean_rel / 1 %)^2"}
-        ctx.fdc_reset()
-
-    # ---- R15: the same plan with a synthetic secondary table (fdc_inputs.add_secondaries)
-    sec_leg = None
-    if world == 1 and rank == 0 and not args.no_secondaries:
-        import fdc_inputs as fi
-        db2, sec = fi.add_secondaries(w.db, 1000 + args.config)
-        if len(sec[1]):
-            arrs2 = [np.ascontiguousarray(a) for a in (db2.dx, db2.dy, db2.dz, db2.dE, db2.E)]
-            ctx.fdc_load_tracks(*arrs2, db2.track_off, db2.bin_first, db2.e_min, db2.e_bin)
-            ctx.fdc_set_secondaries(*sec)
-            ms2, n2 = 0.0, min(5, args.steps)
-            for it in range(2 + n2):
-                flush.fill_(1)
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                torch.cuda.synchronize()
-                e0.record()
-                ctx.fdc_reset()
-                ctx.fdc_run(w.beamlets, first, n_mine, 1, w.seed, flags=flags, dose_gy=dose_d)
-                e1.record()
-                torch.cuda.synchronize()
-                if it >= 2:
-                    ms2 += e0.elapsed_time(e1)
-            st2 = ctx.fdc_get_stats()
-            sec_leg = {"ms_per_step": ms2 / n2, "protons_per_sec": n_mine / (ms2 / n2 * 1e-3), "secondary_tracks": int(len(sec[1])),
-                       "proton_steps": st2["proton_steps"], "deposits": st2["deposits"],
-                       "extra_steps_frac": st2["proton_steps"] / st["proton_steps"] - 1.0,
-                       "extra_time_frac": (ms2 / n2) / (tot_ms / args.steps) - 1.0,
-                       "note": "one synthetic secondary per primary track (tail of another track, 10-40 % of the local energy, "
-                               "10-40 degrees off the parent); k_transport<.,.,SEC>"}
-            ctx.fdc_reset()
-
-    if world > 1:
-        tl = torch.tensor([st["proton_steps"], st["deposits"], st["protons"]], dtype=torch.int64, device=dev)
-        dist.all_reduce(tl)
-        all_steps, all_deps, all_prot = [int(x) for x in tl.tolist()]
-    else:
-        all_steps, all_deps, all_prot = st["proton_steps"], st["deposits"], st["protons"]
+    # ---- the other configs, same process, same flush, same warm-up (N = 1)
+    per_config, sec_leg = None, None
+    if rank == 0 and world == 1 and not args.no_per_config:
+        per_config = {}
+        for c in (1, 2, 3, 4, 5):
+            if c == args.config:
+                continue
+            bc = Bench(c, 1, 0, local, fdc, torch, dist)
+            rc = measure(bc, args, peaks_cache, full=False)
+            per_config["config%d" % c] = dict(workload=bc.w.name, **per_config_entry(rc, args))
+            if c == 2 and not args.no_secondaries:
+                sec_leg = secondaries_leg(bc, args, rc["tot_ms"] / args.steps, rc["st"]["proton_steps"])
+                if sec_leg:
+                    sec_leg["workload"] = bc.w.name
+            bc.close()
+        per_config["config%d" % args.config] = dict(workload=w.name, headline=True, **per_config_entry(res, args))
 
     if rank == 0:
-        hbm_gbs, peak_src = _peaks()
-        n_vox = int(np.prod(w.phantom.hu.shape))
-        # roofline of the dominant kernel (k_transport), rank 0's launches, live CUDA-event durations
-        tr_ms = float(np.mean([k["transport_ms"] for k in ktimes]))
-        # denominators: u64 red rate, uniform random addresses, (i) over an L2-resident buffer and (ii) over a
-        # buffer the size of this grid.  (i) >= (ii); the kernel's deposits are spatially clustered, so on a
-        # grid larger than L2 it can beat (ii) -- the roofline therefore uses (i), the harder ceiling.
-        red_l2 = fdc.fdc_peak_red_u64(local, min(n_vox * 8, 64 << 20), 1 << 30, 0)
-        red_fp = red_l2 if n_vox * 8 <= (64 << 20) else fdc.fdc_peak_red_u64(local, n_vox * 8, 1 << 28, 0)
-        red_peak = max(red_l2, red_fp)
-        # the same microbenchmark with the 32 lanes of a warp in one 32-byte sector group / on one word
-        red_modes = {"lanes_share_4_words": fdc.fdc_peak_red_u64(local, min(n_vox * 8, 64 << 20), 1 << 28, 1) / 1e9,
-                     "lanes_share_1_word": fdc.fdc_peak_red_u64(local, min(n_vox * 8, 64 << 20), 1 << 28, 2) / 1e9,
-                     # every warp of the GPU on a hot set of a few words (config 1: all protons down one column)
-                     "hot_set_256_words": fdc.fdc_peak_red_u64(local, 256 * 8, 1 << 28, 0) / 1e9,
-                     "hot_set_16_words": fdc.fdc_peak_red_u64(local, 16 * 8, 1 << 26, 0) / 1e9}
-        t_track = st["proton_steps"] * STEP_RECORD_BYTES / (hbm_gbs * 1e9)
-        t_atomic = st["deposits"] / red_peak
-        bound_atomic = t_atomic >= t_track
-        roof = {"bound": "l2_atomic" if bound_atomic else "hbm",
-                "achieved": (st["deposits"] / (tr_ms * 1e-3) / 1e9) if bound_atomic else (st["proton_steps"] * STEP_RECORD_BYTES / (tr_ms * 1e-3) / 1e9),
-                "peak": red_peak / 1e9 if bound_atomic else hbm_gbs,
-                "unit": "Gred/s" if bound_atomic else "GB/s",
-                "frac": max(t_track, t_atomic) / (tr_ms * 1e-3),
-                "traffic": None,
-                "kernel": "k_transport", "kernel_ms": tr_ms, "kernel_share_of_step": tr_ms * args.steps / tot_ms * 1.0,
-                "t_track_ms": t_track * 1e3, "t_atomic_ms": t_atomic * 1e3,
-                "hbm": {"achieved_gbs": st["proton_steps"] * STEP_RECORD_BYTES / (tr_ms * 1e-3) / 1e9, "peak_gbs": hbm_gbs, "peak_source": peak_src},
-                "l2_atomic": {"achieved_gred_s": st["deposits"] / (tr_ms * 1e-3) / 1e9, "peak_gred_s": red_peak / 1e9,
-                              "peak_at_grid_footprint_gred_s": red_fp / 1e9, "grid_mib": n_vox * 8 >> 20,
-                              "clustered_peaks_gred_s": red_modes,
-                              "peak_source": "fdc_peak_red_u64 measured in this run: u64 red, uniform random addresses over min(grid, 64 MiB) "
-                                             "(L2-resident); peak_at_grid_footprint is the same over the whole grid"},
-                "algorithmic": {"proton_steps": st["proton_steps"], "deposits": st["deposits"], "bytes_per_step": STEP_RECORD_BYTES,
-                                "note": "deposits = non-zero (step, voxel) shares (R8); the kernel merges the shares one proton leaves in "
-                                        "one voxel into a single red, so it issues fewer reds than deposits"}}
-        traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")     # dram bytes of one ncu --set full capture, per launch
-        if os.path.exists(traffic_file):
-            with open(traffic_file) as f:
-                for line in f.read().splitlines()[1:]:
-                    c = line.split(",")
-                    if len(c) >= 3 and c[0].strip() == str(args.config):
-                        roof["traffic"] = float(c[1])
-                        if args.config != 4:        # config 4's capture is one of two launches per step
-                            # third view: the kernel is bound by instruction issue (4 schedulers x 1 warp
-                            # instruction per clock per SM); instructions from the ncu capture, time and clock live
-                            mhz = (clk or {}).get("sm_mhz") or 1965.0
-                            peak_issue = 148 * 4 * mhz * 1e6
-                            roof["issue"] = {"warp_instructions": float(c[2]), "achieved_ginst_s": float(c[2]) / (tr_ms * 1e-3) / 1e9,
-                                             "peak_ginst_s": peak_issue / 1e9, "frac": float(c[2]) / (tr_ms * 1e-3) / peak_issue,
-                                             "note": "instruction count from profiles/ (ncu smsp__inst_executed.sum), kernel time and SM clock from this run"}
-
-        # cpu baseline: the oracle on a bounded strided sample, this box's host cores
-        cpu = None
-        if world == 1 and not args.no_cpu_baseline:
-            import oracle
-            n_sub = min(args.cpu_sample, w.n_protons)
-            K = max(1, w.n_protons // n_sub)
-            t0 = time.perf_counter()
-            og, ost = oracle.run(w.phantom, w.table, w.db, w.beamlets, w.seed, first=0, n=n_sub, stride=K)
-            dt = time.perf_counter() - t0
-            cpu = {"value": n_sub / dt, "unit": "protons/s", "cores": 1, "kind": "oracle", "host_cores_available": os.cpu_count(),
-                   "steps_per_sec": ost["proton_steps"] / dt,
-                   "sample": "every %d-th proton of %s (%d protons, %.1f s), single thread" % (K, w.name, n_sub, dt)}
-
         out = {"metric": "protons_per_sec", "value": all_prot * args.steps / (tot_ms * 1e-3), "unit": "protons/s", "n_gpus": world,
                "steps": args.steps, "warmup": args.warmup, "ms_per_step": tot_ms / args.steps, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32+u64", "data": "synthetic",
                "steps_per_sec": all_steps * args.steps / (tot_ms * 1e-3), "deposits_per_sec": all_deps * args.steps / (tot_ms * 1e-3),
-               "config": {"workload": w.name, "protons_per_step": all_prot, "protons_per_gpu": per_rank, "grid": list(w.phantom.dims),
-                          "db_tracks": w.db.n_tracks, "db_steps": w.db.n_steps, "beamlets": len(w.beamlets),
-                          "parallelism": "proton ranges x%d, u64 grid all-reduce" % world if world > 1 else "single GPU",
-                          "l2": "flushed between timed steps (512 MiB write)", "timer": "CUDA events per step, max over ranks"},
-               "e2e": {"value": all_prot * args.steps / (e2e_ms * 1e-3), "unit": "protons/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                       "note": "fdc_reset + fdc_run(host beam plan -> pinned host dose grid); phantom and track DB resident"},
-               "e2e_cold": e2e_cold,
-               "gpu_launches": int(sum(k["launches"] for k in ktimes)) + (0 if world == 1 else 0),
-               "wall_s_timed_region": wall, "clocks": clk, "roofline": roof, "cpu_baseline": cpu,
-               "uncertainty": unc, "secondaries": sec_leg, "stats_last_step": st,
+               "config": config, "e2e": res.get("e2e"), "gpu_launches": launches,
+               "wall_s_timed_region": res["wall"], "clocks": res["clk"], "roofline": res["roof"], "cpu_baseline": cpu,
+               "per_config": per_config, "uncertainty": res.get("unc"), "secondaries": sec_leg, "stats_last_step": st,
                "paper_context": "PAPER.md:L114: 184 525 histories/s on one GTX 295 card (other machine, other workload; not a target)"}
         print(json.dumps(out))
-    ctx.fdc_destroy()
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -416,20 +529,30 @@ def run_fdc(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="fdc", choices=["fdc", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[C-1]; 2 is the headline single-GPU workload")
+    ap.add_argument("--config", type=int, default=HEADLINE_CONFIG,
+                    help="BASELINE.json configs[C-1]; 5 (the largest single-GPU configuration) is the headline workload")
     ap.add_argument("--cpu-sample", type=int, default=1_000_000, help="protons of the strided subset the oracle is timed on")
     ap.add_argument("--ref-sample", type=int, default=100_000, help="--impl reference: protons per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-secondaries", action="store_true", help="skip the leg with a synthetic secondary table (R15)")
-    ap.add_argument("--no-squares", action="store_true", help="skip the FDC_TALLY_SQUARES / eq. (2) leg")
-    ap.add_argument("--no-cold", action="store_true", help="skip the e2e_cold leg (context + database re-created from host memory)")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (the other four configs)")
+    ap.add_argument("--no-secondaries", action="store_true", help="skip the leg with a synthetic secondary table (R15; config 2)")
+    ap.add_argument("--no-squares", action="store_true", help="skip the FDC_TALLY_SQUARES / eq. (2) legs")
+    ap.add_argument("--no-cold", action="store_true", help="skip the e2e.cold leg (context + database re-created from host memory)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "fdc":
         print("note: warmup < 3 breaks the timing rules; use for smoke runs only", file=sys.stderr)
-    return run_reference(args) if args.impl == "reference" else run_fdc(args)
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` by hand: re-launch as one rank per GPU, the way the driver does
+        port = 29500 + os.getpid() % 2000
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
+    return run_fdc(args)
 
 
 if __name__ == "__main__":

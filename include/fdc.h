@@ -6,7 +6,9 @@
  *   fdc_create(CT HU grid, voxel spacing, HU -> density / stopping-power / scattering-power table)
  *   fdc_load_tracks(SoA track database binned by incident energy)
  *   fdc_run(beam fields, proton count, seed) -> dose grid
- * plus the paper's uncertainty estimates, phase-space source and gamma index.
+ * plus the final conversion fdc_to_gy as its own call, the paper's uncertainty estimates, phase-space source,
+ * gamma index and profile comparators, and -- in a section of their own at the end -- two
+ * diagnostics that are not part of the method (what the last call did; a trace of where its reductions went).
  * What each call computes is defined rule by rule in DESIGN.md §3 (R1-R15); citations below are
  * PAPER.md line numbers.  Every stage runs in CUDA kernels compiled for sm_100a; there is no CPU
  * fallback (FDC_EARCH on any other device).
@@ -99,8 +101,13 @@ enum {
     FDC_NO_SORT        = 4u,   /* debug: do not group protons by track (same result, slower) */
     FDC_NO_AGGREGATE   = 8u,   /* debug: one atomic per share, no per-voxel merging (same result) */
     FDC_TALLY_SQUARES  = 16u,  /* also tally the sum of squares (second grid; R10) */
-    FDC_REALIGN_START  = 32u   /* rotate a sub-track that starts at a step k0 > first so that step k0 points along
+    FDC_REALIGN_START  = 32u,  /* rotate a sub-track that starts at a step k0 > first so that step k0 points along
                                   the beam (R14); off: the track keeps the deflection it had */
+    FDC_SORT_SPATIAL   = 128u, /* scheduling only (same result): group protons by where they start on the source plane
+                                  instead of by the track they replay; beam plans only */
+    FDC_DIAG_REDS      = 64u   /* diagnostics: run the instrumented instantiation of the transport kernel, which counts
+                                  the 64-bit reductions it sends and records their voxel indices (fdc_trace_reds);
+                                  same tallies, slower; not combinable with FDC_TALLY_SQUARES / FDC_NO_AGGREGATE */
 };
 
 /*
@@ -167,12 +174,26 @@ int fdc_run(fdc_ctx *ctx, const fdc_beamlet *b, uint32_t n_beamlets,
 int fdc_run_phase_space(fdc_ctx *ctx, const fdc_particle *ps, uint64_t n, int ps_is_device_ptr,
                         uint64_t first_id, uint64_t seed, uint32_t flags, float *dose_gy);
 
+/*
+ * Stage 5 on its own ("At the end of the run the energy deposited in each voxel was converted to
+ * absorbed dose by dividing by the mass of the voxel"; R9): the grid as it stands -> nx*ny*nz floats in
+ * Gy, device memory or (is_device_ptr = 0; synchronises) host memory.  fdc_run's dose_gy argument is this call
+ * appended to the transport; a multi-GPU run calls it once after the grids have been summed.
+ */
+int fdc_to_gy(fdc_ctx *ctx, float *dose_gy, int is_device_ptr);
+
 /* Copy out the raw fixed-point grid (nx*ny*nz u64, quanta of 2^-24 MeV). */
 int fdc_get_edep_fixed(fdc_ctx *ctx, uint64_t *grid_out, int is_device_ptr);
 
 /* Overwrite the raw fixed-point grid, e.g. with the sum over GPUs after an integer all-reduce (the
  * paper's "absorbed dose from both threads was combined"); counters are unchanged. */
 int fdc_set_edep_fixed(fdc_ctx *ctx, const uint64_t *grid_in, int is_device_ptr);
+
+/* The context's own device arrays, BORROWED (valid until fdc_destroy; owned by the library): the u64 energy grid
+ * and, if one exists (else NULL), the sum-of-squares grid -- so that the integer all-reduce over GPUs
+ * can run in place on the caller's stream instead of through get / set copies.  The caller must
+ * order its work against the context's stream. */
+int fdc_edep_device_ptr(fdc_ctx *ctx, uint64_t **edep, uint64_t **squares /* may be NULL */);
 
 /*
  * Sum-of-squares tally ("a second tallying array ... the sum of the squares of the
@@ -233,20 +254,54 @@ void fdc_destroy(fdc_ctx *ctx);
 const char *fdc_strerror(int code);
 const char *fdc_last_error(const fdc_ctx *ctx);      /* text of the last FDC_ECUDA / FDC_EINVAL */
 
-/* Device time in milliseconds of the kernels of the most recent fdc_run, measured with CUDA events
- * on the context's stream: [0] whole call on the device, [1] transport+deposit kernels only,
- * [2] sampling-key + sort kernels, [3] Gy kernel.  launches = kernels launched by that call.
- * Synchronises the stream. */
-int fdc_last_timing(fdc_ctx *ctx, float ms[4], uint32_t *launches);
-
 /*
- * Roofline denominator: measured throughput of 64-bit reductions (`red.global.add.u64`, the
- * deposit instruction) over a buffer of footprint_bytes on `device`: n_ops operations from a
- * saturating grid, addresses from an integer hash of the operation index (the footprint is rounded
- * down to a power of two).  mode 0: uniform over the footprint; 1: the 32 lanes of a warp fall in one 32-byte sector group (4 distinct words);
- * 2: all lanes of a warp hit one word.  Returns operations per second in *ops_per_s.
+ * Profile comparators (Fig. 2-3; R16, R17).
+ *
+ * fdc_profile: the paper's depth and cross-field profiles, "calculated along a five voxel thick line" (L104).
+ * values: DEVICE array of nx*ny*nz floats (a dose grid), or NULL for the context's own energy grid in MeV (Fig. 2
+ * plots deposited energy).  The line runs along `axis` (0 = x, 1 = y, 2 = z) through the voxel whose indices on
+ * the other two axes (a = the lower-numbered one, b = the other) are (fixed_a, fixed_b); it is thickened to the
+ * bundle of columns |a - fixed_a| <= half_width_a, |b - fixed_b| <= half_width_b clipped to the grid (2, 2 = five
+ * voxels thick; 2, 0 = a five-voxel slab), and out[k], k < n_axis, is the mean over the bundle (f64; summed b
+ * outer, a inner, then divided by the number of columns).  out: n_axis doubles, host (synchronises) or device.
+ * FDC_EINVAL if the line lies outside the grid.
+ *
+ * fdc_rms_diff: "the difference between the ... doses for each voxel ... divided by the maximum [reference] voxel
+ * dose has a RMS value of 0.5 %" (L108): *rms_over_max = sqrt(mean over ALL voxels of ((eval - ref) * (1 / max
+ * ref))^2), f64 per voxel, summed exactly in 128-bit fixed point (quantum 2^-64: independent of the order of the
+ * additions).  Both arrays DEVICE, nx*ny*nz floats.  *max_ref (may be NULL) receives the maximum.  Synchronises.
  */
-int fdc_peak_red_u64(int device, uint64_t footprint_bytes, uint64_t n_ops, int mode, double *ops_per_s);
+int fdc_profile(fdc_ctx *ctx, const float *values, int axis, int fixed_a, int fixed_b, int half_width_a, int half_width_b,
+                double *out, int out_is_device_ptr);
+int fdc_rms_diff(fdc_ctx *ctx, const float *dose_ref, const float *dose_eval, double *rms_over_max, double *max_ref);
+
+/* ------------------------------------------------------------------------------------------------------------
+ * Diagnostics.  NOT part of the method and not among the calls SURVEY §8(b) lists: they report what the library
+ * did, for bench.py's timing split, its end-to-end byte counts and its contention-limited roofline ceiling.  The
+ * roofline microbenchmarks themselves live in a separate library (csrc/bench_peaks.cu -> libfdcpeaks.so).
+ * ------------------------------------------------------------------------------------------------------------ */
+
+/* What the most recent fdc_run / fdc_run_phase_space did, together with any fdc_to_gy calls made since (their
+ * kernel and copy are added to launches, ms_gy, d2h_bytes; ms_total then spans from the start of the run to the
+ * end of the last conversion).  Times are device times from CUDA events on the context's stream.  Synchronises. */
+typedef struct {
+    float ms_total;          /* whole call on the device */
+    float ms_transport;      /* transport + deposit kernels */
+    float ms_sort;           /* sampling-key + grouping kernels */
+    float ms_gy;             /* Gy kernel (and the device-to-host copy of the dose grid, if any) */
+    uint32_t launches;       /* kernels launched by the call */
+    uint32_t reserved;
+    uint64_t h2d_bytes;      /* bytes the call copied from host memory to the device (0 when the plan was cached) */
+    uint64_t d2h_bytes;      /* bytes it copied back */
+    uint64_t reds_sent;      /* FDC_DIAG_REDS runs since the last fdc_reset: 64-bit reductions actually sent */
+    uint64_t reds_traced;    /* of those of the last call, how many are in the trace buffer */
+} fdc_call_info;
+int fdc_last_call_info(fdc_ctx *ctx, fdc_call_info *out);
+
+/* Set (or, with NULL / 0, remove) a DEVICE buffer of `capacity` uint32 that FDC_DIAG_REDS runs fill with the voxel
+ * index of every reduction they send, in the order the hardware serialises the appends; each such run starts
+ * again at entry 0.  Borrowed until replaced. */
+int fdc_trace_reds(fdc_ctx *ctx, uint32_t *trace_dev, uint64_t capacity);
 
 #ifdef __cplusplus
 }

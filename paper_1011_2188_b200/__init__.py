@@ -21,12 +21,16 @@ FDC_NO_SORT = 4
 FDC_NO_AGGREGATE = 8
 FDC_TALLY_SQUARES = 16
 FDC_REALIGN_START = 32
+FDC_DIAG_REDS = 64
+FDC_SORT_SPATIAL = 128
 
 FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH = 0, -1, -2, -3, -4, -5, -6
 
-EXPORTS = ["fdc_create", "fdc_load_tracks", "fdc_run", "fdc_get_edep_fixed", "fdc_set_edep_fixed", "fdc_get_stats", "fdc_reset",
-           "fdc_destroy", "fdc_strerror", "fdc_last_error", "fdc_last_timing", "fdc_peak_red_u64",
-           "fdc_get_sq_fixed", "fdc_set_sq_fixed", "fdc_uncertainty_history", "fdc_uncertainty_batch", "fdc_run_phase_space", "fdc_gamma_index", "fdc_set_secondaries"]
+EXPORTS = ["fdc_create", "fdc_load_tracks", "fdc_run", "fdc_to_gy", "fdc_get_edep_fixed", "fdc_set_edep_fixed", "fdc_edep_device_ptr",
+           "fdc_get_stats", "fdc_reset", "fdc_destroy", "fdc_strerror", "fdc_last_error",
+           "fdc_get_sq_fixed", "fdc_set_sq_fixed", "fdc_uncertainty_history", "fdc_uncertainty_batch", "fdc_run_phase_space", "fdc_gamma_index",
+           "fdc_profile", "fdc_rms_diff", "fdc_set_secondaries",
+           "fdc_last_call_info", "fdc_trace_reds"]          # the last two: diagnostics (include/fdc.h)
 
 BEAMLET_DTYPE = np.dtype([("origin", "<f4", 3), ("e1", "<f4", 3), ("e2", "<f4", 3), ("dir", "<f4", 3),
                           ("energy_mev", "<f4"), ("spot_u_mm", "<f4"), ("spot_v_mm", "<f4"),
@@ -46,6 +50,12 @@ class _TrackDB(ctypes.Structure):
                 ("E", ctypes.c_void_p), ("n_steps", ctypes.c_uint64), ("track_off", ctypes.c_void_p),
                 ("n_tracks", ctypes.c_uint32), ("bin_first", ctypes.c_void_p), ("n_bins", ctypes.c_uint32),
                 ("e_min_mev", ctypes.c_float), ("e_bin_mev", ctypes.c_float)]
+
+
+class _CallInfo(ctypes.Structure):
+    _fields_ = [("ms_total", ctypes.c_float), ("ms_transport", ctypes.c_float), ("ms_sort", ctypes.c_float), ("ms_gy", ctypes.c_float),
+                ("launches", ctypes.c_uint32), ("reserved", ctypes.c_uint32), ("h2d_bytes", ctypes.c_uint64), ("d2h_bytes", ctypes.c_uint64),
+                ("reds_sent", ctypes.c_uint64), ("reds_traced", ctypes.c_uint64)]
 
 
 class _Stats(ctypes.Structure):
@@ -85,8 +95,18 @@ def lib():
         L.fdc_strerror.argtypes = [i32]
         L.fdc_last_error.restype = ctypes.c_char_p
         L.fdc_last_error.argtypes = [vp]
-        L.fdc_last_timing.restype = i32
-        L.fdc_last_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float * 4), ctypes.POINTER(u32)]
+        L.fdc_last_call_info.restype = i32
+        L.fdc_last_call_info.argtypes = [vp, ctypes.POINTER(_CallInfo)]
+        L.fdc_trace_reds.restype = i32
+        L.fdc_trace_reds.argtypes = [vp, vp, u64]
+        L.fdc_to_gy.restype = i32
+        L.fdc_to_gy.argtypes = [vp, vp, i32]
+        L.fdc_edep_device_ptr.restype = i32
+        L.fdc_edep_device_ptr.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp)]
+        L.fdc_profile.restype = i32
+        L.fdc_profile.argtypes = [vp, vp, i32, i32, i32, i32, i32, vp, i32]
+        L.fdc_rms_diff.restype = i32
+        L.fdc_rms_diff.argtypes = [vp, vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
         for f in (L.fdc_get_sq_fixed, L.fdc_set_sq_fixed):
             f.restype = i32
             f.argtypes = [vp, vp, i32]
@@ -100,8 +120,6 @@ def lib():
         L.fdc_uncertainty_history.argtypes = [vp, u64, vp, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
         L.fdc_uncertainty_batch.restype = i32
         L.fdc_uncertainty_batch.argtypes = [vp, vp, i32, u64, vp, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
-        L.fdc_peak_red_u64.restype = i32
-        L.fdc_peak_red_u64.argtypes = [i32, u64, u64, i32, ctypes.POINTER(ctypes.c_double)]
         _lib = L
     return _lib
 
@@ -121,12 +139,12 @@ def _is_device(x):
     return (not isinstance(x, np.ndarray)) and x.is_cuda
 
 
-def fdc_peak_red_u64(device: int, footprint_bytes: int, n_ops: int, mode: int = 0) -> float:
-    out = ctypes.c_double(0.0)
-    rc = lib().fdc_peak_red_u64(device, footprint_bytes, n_ops, mode, ctypes.byref(out))
-    if rc != 0:
-        raise FdcError(rc, lib().fdc_strerror(rc).decode())
-    return out.value
+class _DeviceArray:
+    """A borrowed device array as a __cuda_array_interface__ object (so torch can alias it without a copy)."""
+
+    def __init__(self, ptr, shape, typestr, owner):
+        self.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": typestr, "data": (int(ptr), False), "version": 3, "strides": None}
+        self._owner = owner
 
 
 class Fdc:
@@ -201,6 +219,37 @@ class Fdc:
             flags |= FDC_DOSE_TO_HOST
         self._check(self._lib.fdc_run_phase_space(self._h, _ptr(ps), n, dev, int(first_id), int(seed), flags, _ptr(dose_gy)))
 
+    def fdc_to_gy(self, dose_gy):
+        """Stage 5 alone: the grid as it stands -> Gy into a CUDA float32 tensor or a host float32 array."""
+        self._check(self._lib.fdc_to_gy(self._h, _ptr(dose_gy), 1 if _is_device(dose_gy) else 0))
+
+    def fdc_edep_device_ptr(self):
+        """The context's own grids as torch int64 CUDA tensors aliasing the library's memory (borrowed: valid until
+        fdc_destroy): (energy grid, squares grid or None).  For the in-place all-reduce over GPUs."""
+        e = ctypes.c_void_p(None); q = ctypes.c_void_p(None)
+        self._check(self._lib.fdc_edep_device_ptr(self._h, ctypes.byref(e), ctypes.byref(q)))
+        torch = self._torch
+        mk = lambda p: torch.as_tensor(_DeviceArray(p, self.shape, "<i8", self), device=torch.device("cuda", self.device))
+        return mk(e.value), (mk(q.value) if q.value else None)
+
+    def fdc_profile(self, values, axis, fixed_a, fixed_b, half_width_a=2, half_width_b=2, out=None):
+        """values: CUDA float32 tensor [nz,ny,nx] or None (the energy grid, MeV).  Returns the profile (host float64
+        numpy array of n_axis entries, or `out`, a CUDA float64 tensor, filled)."""
+        n_axis = self.shape[2 - axis]
+        if out is None:
+            out = np.empty(n_axis, dtype=np.float64)
+        assert values is None or _is_device(values)
+        self._check(self._lib.fdc_profile(self._h, _ptr(values), int(axis), int(fixed_a), int(fixed_b), int(half_width_a), int(half_width_b),
+                                          _ptr(out), 1 if _is_device(out) else 0))
+        return out
+
+    def fdc_rms_diff(self, dose_ref, dose_eval):
+        """CUDA float32 tensors [nz,ny,nx].  Returns (rms of (eval - ref) / max(ref) over all voxels, max(ref))."""
+        assert _is_device(dose_ref) and _is_device(dose_eval)
+        r = ctypes.c_double(0.0); m = ctypes.c_double(0.0)
+        self._check(self._lib.fdc_rms_diff(self._h, _ptr(dose_ref), _ptr(dose_eval), ctypes.byref(r), ctypes.byref(m)))
+        return r.value, m.value
+
     def fdc_get_edep_fixed(self, out=None):
         """Raw grid; out: CUDA int64 tensor, or None -> new host numpy uint64 [nz,ny,nx]."""
         if out is None:
@@ -258,11 +307,22 @@ class Fdc:
     def fdc_reset(self):
         self._check(self._lib.fdc_reset(self._h))
 
-    def fdc_last_timing(self) -> dict:
-        ms = (ctypes.c_float * 4)()
-        n = ctypes.c_uint32(0)
-        self._check(self._lib.fdc_last_timing(self._h, ctypes.byref(ms), ctypes.byref(n)))
-        return {"total_ms": ms[0], "transport_ms": ms[1], "sort_ms": ms[2], "gy_ms": ms[3], "launches": int(n.value)}
+    def fdc_last_call_info(self) -> dict:
+        """Diagnostics: device times, launches and host<->device bytes of the most recent run / fdc_to_gy."""
+        ci = _CallInfo()
+        self._check(self._lib.fdc_last_call_info(self._h, ctypes.byref(ci)))
+        return {"total_ms": ci.ms_total, "transport_ms": ci.ms_transport, "sort_ms": ci.ms_sort, "gy_ms": ci.ms_gy, "launches": int(ci.launches),
+                "h2d_bytes": int(ci.h2d_bytes), "d2h_bytes": int(ci.d2h_bytes), "reds_sent": int(ci.reds_sent), "reds_traced": int(ci.reds_traced)}
+
+    def fdc_trace_reds(self, trace=None):
+        """Diagnostics: a CUDA int32/uint32 tensor that FDC_DIAG_REDS runs fill with voxel indices (None removes it)."""
+        if trace is None:
+            self._trace = None
+            self._check(self._lib.fdc_trace_reds(self._h, None, 0))
+        else:
+            assert trace.is_cuda and trace.is_contiguous() and trace.element_size() == 4
+            self._trace = trace
+            self._check(self._lib.fdc_trace_reds(self._h, _ptr(trace), trace.numel()))
 
     def fdc_destroy(self):
         if self._h:

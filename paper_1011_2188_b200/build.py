@@ -1,4 +1,5 @@
-"""Build paper_1011_2188_b200/libfdc.so in-tree with nvcc for sm_100a (cross-compiles without a GPU)."""
+"""Build paper_1011_2188_b200/libfdc.so (the method) and libfdcpeaks.so (bench.py's roofline microbenchmarks) in-tree
+with nvcc for sm_100a (cross-compiles without a GPU)."""
 from __future__ import annotations
 
 import os
@@ -9,6 +10,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "fdc.cu")
 HDR = os.path.join(os.path.dirname(HERE), "include", "fdc.h")
 LIB = os.path.join(HERE, "libfdc.so")
+PEAKS_SRC = os.path.join(HERE, "csrc", "bench_peaks.cu")
+PEAKS_LIB = os.path.join(HERE, "libfdcpeaks.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               # arithmetic contract: no contraction, IEEE div/sqrt, denormals kept
@@ -24,6 +27,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
         cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp, SRC]
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
+    if force or not os.path.exists(PEAKS_LIB) or os.path.getmtime(PEAKS_LIB) < os.path.getmtime(PEAKS_SRC):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        tmp = PEAKS_LIB + ".tmp.%d" % os.getpid()
+        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+                               "-Xcompiler", "-fPIC", "-shared", "-o", tmp, PEAKS_SRC])
+        os.replace(tmp, PEAKS_LIB)
     return LIB
 
 

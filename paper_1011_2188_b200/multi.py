@@ -23,17 +23,28 @@ def allreduce_sum_int64(t):
     return t
 
 
-def allreduce_edep(ctx, scratch):
-    """Replace ctx's grid by the sum over ranks.  scratch: CUDA int64 tensor shaped like the grid."""
-    ctx.fdc_get_edep_fixed(scratch)
-    allreduce_sum_int64(scratch)
-    ctx.fdc_set_edep_fixed(scratch)
+def allreduce_edep(ctx, squares=False):
+    """Replace ctx's energy grid (and, with squares=True, its sum-of-squares grid: eq. (2)'s sums run over the
+    histories of all ranks) by the sum over ranks, IN PLACE on the library's own device arrays
+    (fdc_edep_device_ptr): one all-reduce per grid, no staging copies.  The tensors alias the context's memory and
+    the collective runs on the stream the context was created on (torch's current stream), after the transport
+    kernels queued there."""
+    e, q = ctx.fdc_edep_device_ptr()
+    allreduce_sum_int64(e)
+    if squares and q is not None:
+        allreduce_sum_int64(q)
 
 
-def allreduce_squares(ctx, scratch):
-    """Same for the sum-of-squares grid (FDC_TALLY_SQUARES): eq. (2)'s sums run over the histories of
-    all ranks, and both sums are integers, so the N-GPU uncertainty map equals the 1-GPU one."""
-    ctx.fdc_get_sq_fixed(scratch)
-    allreduce_sum_int64(scratch)
-    ctx.fdc_set_sq_fixed(scratch)
-
+def sharded_step(ctx, beamlets, first, n_mine, seed, flags, dose_out, world):
+    """One step of the hot path on this rank: zero, transport this rank's proton range [first, first + n_mine),
+    and -- for world > 1 -- sum the grids over ranks in place, then convert to Gy (each GPU unit
+    handles its histories; "the absorbed dose from both threads was combined" at the end).  With world == 1 the Gy
+    conversion rides on fdc_run itself.  dose_out: CUDA tensor or host array (then the call synchronises)."""
+    ctx.fdc_reset()
+    if world == 1:
+        ctx.fdc_run(beamlets, first, n_mine, 1, seed, flags=flags, dose_gy=dose_out)
+        return
+    ctx.fdc_run(beamlets, first, n_mine, 1, seed, flags=flags)
+    allreduce_edep(ctx, squares=bool(flags & 16))          # 16 = FDC_TALLY_SQUARES
+    if dose_out is not None:
+        ctx.fdc_to_gy(dose_out)
