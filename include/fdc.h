@@ -105,6 +105,10 @@ enum {
                                   the beam (R14); off: the track keeps the deflection it had */
     FDC_SORT_SPATIAL   = 128u, /* scheduling only (same result): group protons by where they start on the source plane
                                   instead of by the track they replay; beam plans only */
+    FDC_PRIVATE_TALLY  = 512u, /* scheduling only (same result): route the reductions through a per-CTA table in shared memory
+                                  that is emptied into the grid every few rounds (north_star (4)); meant to be
+                                  used with FDC_SORT_SPATIAL; ignored with FDC_TALLY_SQUARES / FDC_NO_AGGREGATE */
+    FDC_NO_LAT         = 256u, /* debug: do not use the latency-optimised instantiation for small plans (same result) */
     FDC_DIAG_REDS      = 64u   /* diagnostics: run the instrumented instantiation of the transport kernel, which counts
                                   the 64-bit reductions it sends and records their voxel indices (fdc_trace_reds);
                                   same tallies, slower; not combinable with FDC_TALLY_SQUARES / FDC_NO_AGGREGATE */

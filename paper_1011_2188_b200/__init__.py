@@ -23,6 +23,8 @@ FDC_TALLY_SQUARES = 16
 FDC_REALIGN_START = 32
 FDC_DIAG_REDS = 64
 FDC_SORT_SPATIAL = 128
+FDC_NO_LAT = 256
+FDC_PRIVATE_TALLY = 512
 
 FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH = 0, -1, -2, -3, -4, -5, -6
 

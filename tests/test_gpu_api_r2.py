@@ -120,7 +120,7 @@ def test_call_info_counts_the_copies(fdc, wl3_small):
     w = wl3_small
     ctx = make_ctx(fdc, w)
     nb = len(w.beamlets)
-    plan_bytes = nb * 72 + (nb + 1) * 8
+    plan_bytes = nb * (72 + 20) + (nb + 1) * 8          # beamlets + their sort-key records + prefix sums
     ctx.fdc_run(w.beamlets, 0, 100, 1, w.seed)
     a = ctx.fdc_last_call_info()
     assert a["h2d_bytes"] == plan_bytes and a["d2h_bytes"] == 0 and a["launches"] == 6 and a["transport_ms"] > 0
@@ -130,7 +130,7 @@ def test_call_info_counts_the_copies(fdc, wl3_small):
     dose = np.zeros(w.phantom.hu.shape, dtype=np.float32)
     ctx.fdc_run(bl2, 200, 100, 1, w.seed, dose_gy=dose)
     c = ctx.fdc_last_call_info()
-    assert c["h2d_bytes"] == plan_bytes + 80 and c["d2h_bytes"] == dose.nbytes and c["launches"] == 7
+    assert c["h2d_bytes"] == plan_bytes + 100 and c["d2h_bytes"] == dose.nbytes and c["launches"] == 7
     ctx.fdc_destroy()
 
 

@@ -46,7 +46,7 @@ def check_against_oracle(fdc, w, ctx=None, flags=1, first=0, n=None, stride=1, s
     ctx.fdc_run(w.beamlets, first, n, stride, seed, flags=flags, dose_gy=dose)
     g = ctx.fdc_get_edep_fixed()
     st = ctx.fdc_get_stats()
-    og, ost = oracle.run(w.phantom, w.table, w.db, w.beamlets, seed, first=first, n=n, stride=stride, flags=flags & 33)
+    og, ost = oracle.run(w.phantom, w.table, w.db, w.beamlets, seed, first=first, n=n, stride=stride, flags=flags & 33)   # 33: the flags that change the result
     assert np.array_equal(g, og), "fixed-point grid differs: %d voxels, sum %d vs %d" % (
         int((g != og).sum()), int(g.sum(dtype=np.uint64)), int(og.sum(dtype=np.uint64)))
     for k in STAT_KEYS:
@@ -80,6 +80,13 @@ def test_flags_and_ranges(fdc, wl3_small):
     g_nosort, _ = check_against_oracle(fdc, w, ctx, flags=1 | fdc.FDC_NO_SORT)
     g_noagg, _ = check_against_oracle(fdc, w, ctx, flags=1 | fdc.FDC_NO_AGGREGATE)
     assert np.array_equal(g_sorted, g_nosort) and np.array_equal(g_sorted, g_noagg)
+    # scheduling variants: the big-plan instantiation on this small plan; grouping by start position with
+    # the CTA-private tally; both at once -- the integers cannot change
+    sp, pt = fdc.FDC_SORT_SPATIAL, fdc.FDC_PRIVATE_TALLY
+    for fl in (1 | fdc.FDC_NO_LAT, 1 | sp, 1 | sp | fdc.FDC_NO_LAT, 1 | sp | pt, sp | pt, 1 | pt, 1 | fdc.FDC_NO_SORT | fdc.FDC_NO_LAT):
+        g_v, _ = check_against_oracle(fdc, w, ctx, flags=fl)
+        if fl & 1:
+            assert np.array_equal(g_sorted, g_v), fl
     check_against_oracle(fdc, w, ctx, flags=0)                                   # azimuth off
     check_against_oracle(fdc, w, ctx, first=7, n=300, stride=13)                 # strided subset
     check_against_oracle(fdc, w, ctx, first=4000, n=704)                         # tail range
@@ -575,6 +582,12 @@ def test_random_degenerate_worlds(fdc):
         ctx = make_ctx(fdc, w)
         flags = int(rng.choice([0, 1, 1 | ra, 1 | fdc.FDC_NO_SORT, 1 | fdc.FDC_NO_AGGREGATE]))
         check_against_oracle(fdc, w, ctx, flags=flags)
+        # every world also through the other instantiations of the kernel (small plans take the latency-optimised one by
+        # default): the big-plan one, and the one with grouping by start position + CTA-private tally
+        check_against_oracle(fdc, w, ctx, flags=(flags & ~fdc.FDC_NO_AGGREGATE) | fdc.FDC_NO_LAT)
+        if case % 2 == 0:
+            check_against_oracle(fdc, w, ctx, flags=(flags & ~(fdc.FDC_NO_AGGREGATE | fdc.FDC_NO_SORT)) | fdc.FDC_SORT_SPATIAL |
+                                 (fdc.FDC_PRIVATE_TALLY if case % 4 == 0 else 0))
         if case % 5 == 1:                             # the same world entered from a random phase-space array
             n = 150
             ext = np.array(w.phantom.dims) * np.array(w.phantom.spacing)

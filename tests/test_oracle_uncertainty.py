@@ -151,3 +151,31 @@ def test_uncertainty_scaling_and_batch_agreement():
     ub, _ = oracle.mean_uncertainty(mb / N, sb / N, rho)
     uh, _ = oracle.mean_uncertainty(mh, sh, rho)
     assert ub / uh == pytest.approx(1.0, rel=0.35)       # 5 degrees of freedom per voxel, averaged over tens of voxels
+
+
+@pytest.mark.parametrize("cfg,n,tpb", [(2, 20000, 300), (3, 23520, 50)])
+def test_by_visit_gap_is_measured_with_and_without_secondaries(cfg, n, tpb):
+    """DESIGN.md R10 / reading A23, measured: how far the per-stay tally (what the fast kernel squares) falls short of
+    eq. (2)'s per-history D_i, on reduced configs 2 and 3, primaries only and with the synthetic
+    secondaries of fdc_inputs.add_secondaries (parent and secondary both deposit in the branch voxel and are squared
+    separately).  Bounds enforced: primaries only, gap <= 1e-3 of the tally and the mean relative uncertainty
+     changes by <= 1e-3 of itself; with secondaries, gap <= 6 % and the mean relative uncertainty is low
+    by <= 4 %.  by_visit <= by_history voxel by voxel in every case (a sum of squares of parts never exceeds the square
+    of the sum)."""
+    import fdc_inputs as fi
+    w = fi.workload(cfg, n_protons=n, tracks_per_bin=tpb)
+    rho = oracle.density(w.phantom, w.table)
+    res = {}
+    for with_sec in (False, True):
+        if with_sec:
+            db2, sec = fi.add_secondaries(w.db, 1000 + cfg)
+            assert len(sec[1]) > 0
+            g, sv, sh, st = oracle.run_secondaries(w.phantom, w.table, db2, sec, w.beamlets, w.seed, squares=True)
+        else:
+            g, sv, sh, st = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed)
+        assert np.all(sv <= sh)
+        gap = float(sh.sum() - sv.sum()) / float(sh.sum())
+        rel = [oracle.mean_uncertainty(*oracle.sigma_history(g, sq, n), rho)[0] for sq in (sv, sh)]
+        res[with_sec] = (gap, rel[0] / rel[1])
+    assert 0.0 <= res[False][0] <= 1e-3 and 1.0 - 1e-3 <= res[False][1] <= 1.0
+    assert 0.005 <= res[True][0] <= 0.06 and 0.96 <= res[True][1] <= 1.0
