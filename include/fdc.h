@@ -108,7 +108,15 @@ enum {
     FDC_PRIVATE_TALLY  = 512u, /* scheduling only (same result): route the reductions through a per-CTA table in shared memory
                                   that is emptied into the grid every few rounds (north_star (4)); meant to be
                                   used with FDC_SORT_SPATIAL; ignored with FDC_TALLY_SQUARES / FDC_NO_AGGREGATE */
-    FDC_NO_LAT         = 256u, /* debug: do not use the latency-optimised instantiation for small plans (same result) */
+    FDC_NO_LAT         = 256u, /* debug: run a small plan (at most one wave of thread blocks) through the same instantiation as a
+                                  large one; by default it runs with the CTA-private tally of FDC_PRIVATE_TALLY (same result) */
+    FDC_MAT_TILED      = 2048u,/* scheduling only (same result): the transport kernel reads the material of the voxel ahead from the
+                                  library's tiled copy of the material grid (4 x 4 x 1 voxels per 32-byte sector) ... */
+    FDC_MAT_LINEAR     = 4096u,/* ... or from the x-fastest one.  Default: tiled iff the material and energy grids together
+                                  (10 bytes per voxel) exceed the device's L2 cache */
+    FDC_WARP_AGGREGATE = 1024u,/* scheduling only (same result): a small plan runs the latency-oriented instantiation that sums the
+                                  shares of the lanes leaving the same voxel over the warp and sends one reduction per distinct
+                                  voxel (north_star (4)), instead of the CTA-private tally; ignored for larger plans */
     FDC_DIAG_REDS      = 64u   /* diagnostics: run the instrumented instantiation of the transport kernel, which counts
                                   the 64-bit reductions it sends and records their voxel indices (fdc_trace_reds);
                                   same tallies, slower; not combinable with FDC_TALLY_SQUARES / FDC_NO_AGGREGATE */

@@ -25,6 +25,9 @@ FDC_DIAG_REDS = 64
 FDC_SORT_SPATIAL = 128
 FDC_NO_LAT = 256
 FDC_PRIVATE_TALLY = 512
+FDC_WARP_AGGREGATE = 1024
+FDC_MAT_TILED = 2048
+FDC_MAT_LINEAR = 4096
 
 FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH = 0, -1, -2, -3, -4, -5, -6
 

@@ -80,10 +80,12 @@ def test_flags_and_ranges(fdc, wl3_small):
     g_nosort, _ = check_against_oracle(fdc, w, ctx, flags=1 | fdc.FDC_NO_SORT)
     g_noagg, _ = check_against_oracle(fdc, w, ctx, flags=1 | fdc.FDC_NO_AGGREGATE)
     assert np.array_equal(g_sorted, g_nosort) and np.array_equal(g_sorted, g_noagg)
-    # scheduling variants: the big-plan instantiation on this small plan; grouping by start position with
-    # the CTA-private tally; both at once -- the integers cannot change
+    # scheduling variants: this small plan runs with the CTA-private tally by default; the big-plan instantiation
+    # (FDC_NO_LAT), the warp-aggregating one (FDC_WARP_AGGREGATE), grouping by start position -- the integers cannot change
     sp, pt = fdc.FDC_SORT_SPATIAL, fdc.FDC_PRIVATE_TALLY
-    for fl in (1 | fdc.FDC_NO_LAT, 1 | sp, 1 | sp | fdc.FDC_NO_LAT, 1 | sp | pt, sp | pt, 1 | pt, 1 | fdc.FDC_NO_SORT | fdc.FDC_NO_LAT):
+    wa, mt, ml = fdc.FDC_WARP_AGGREGATE, fdc.FDC_MAT_TILED, fdc.FDC_MAT_LINEAR
+    for fl in (1 | mt, 1 | ml, 1 | mt | fdc.FDC_NO_LAT, 1 | mt | fdc.FDC_NO_SORT, 1 | mt | fdc.FDC_NO_AGGREGATE, 1 | mt | fdc.FDC_TALLY_SQUARES, 1 | fdc.FDC_NO_LAT, 1 | wa, 1 | sp, 1 | sp | wa, 1 | sp | fdc.FDC_NO_LAT, 1 | sp | pt, sp | pt, 1 | pt, 1 | fdc.FDC_NO_SORT | fdc.FDC_NO_LAT,
+               1 | fdc.FDC_NO_SORT | wa):
         g_v, _ = check_against_oracle(fdc, w, ctx, flags=fl)
         if fl & 1:
             assert np.array_equal(g_sorted, g_v), fl
@@ -582,9 +584,12 @@ def test_random_degenerate_worlds(fdc):
         ctx = make_ctx(fdc, w)
         flags = int(rng.choice([0, 1, 1 | ra, 1 | fdc.FDC_NO_SORT, 1 | fdc.FDC_NO_AGGREGATE]))
         check_against_oracle(fdc, w, ctx, flags=flags)
-        # every world also through the other instantiations of the kernel (small plans take the latency-optimised one by
-        # default): the big-plan one, and the one with grouping by start position + CTA-private tally
+        # every world also through the other instantiations of the kernel (small plans take the CTA-private tally by
+        # default): the big-plan one, the warp-aggregating one, and grouping by start position with and without the private tally
         check_against_oracle(fdc, w, ctx, flags=(flags & ~fdc.FDC_NO_AGGREGATE) | fdc.FDC_NO_LAT)
+        check_against_oracle(fdc, w, ctx, flags=(flags & ~fdc.FDC_NO_AGGREGATE) | fdc.FDC_WARP_AGGREGATE)
+        # and with the material read from the tiled copy of the grid (default only for grids beyond L2), big-plan and default kernels
+        check_against_oracle(fdc, w, ctx, flags=flags | fdc.FDC_MAT_TILED | (fdc.FDC_NO_LAT if case % 2 else 0))
         if case % 2 == 0:
             check_against_oracle(fdc, w, ctx, flags=(flags & ~(fdc.FDC_NO_AGGREGATE | fdc.FDC_NO_SORT)) | fdc.FDC_SORT_SPATIAL |
                                  (fdc.FDC_PRIVATE_TALLY if case % 4 == 0 else 0))
@@ -639,7 +644,9 @@ def test_secondaries_bit_exact(fdc):
         w = fi.Workload("sec", ph, table_uniform(1.0), db, fi.single_beamlet((31.0, 33.0, 1.0), e0, 1.5, 400), 400, 5)
         ctx = make_ctx(fdc, w)
         ctx.fdc_set_secondaries(*sec)
-        for flags in (1, 0, 1 | sq, 1 | fdc.FDC_NO_SORT, 1 | fdc.FDC_NO_AGGREGATE, 1 | fdc.FDC_REALIGN_START):
+        mt = fdc.FDC_MAT_TILED
+        for flags in (1, 0, 1 | sq, 1 | fdc.FDC_NO_SORT, 1 | fdc.FDC_NO_AGGREGATE, 1 | fdc.FDC_REALIGN_START, 1 | mt, 1 | mt | sq, 1 | mt | fdc.FDC_NO_LAT,
+                      1 | mt | fdc.FDC_NO_AGGREGATE):
             gpu_vs_oracle(ctx, w, db, sec, flags)
         ctx.fdc_set_secondaries(np.zeros(db.n_tracks + 1, np.uint32), [], [])          # removed: the plain run again
         ctx.fdc_reset(); ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed)
@@ -659,7 +666,7 @@ def test_secondaries_bit_exact(fdc):
         ctx = make_ctx(fdc, w)
         if len(sec2[1]):
             ctx.fdc_set_secondaries(*sec2)
-        gpu_vs_oracle(ctx, w, db2, sec2, int(rng.choice([0, 1, 1 | sq, 1 | fdc.FDC_REALIGN_START, 1 | fdc.FDC_NO_AGGREGATE])))
+        gpu_vs_oracle(ctx, w, db2, sec2, int(rng.choice([0, 1, 1 | sq, 1 | fdc.FDC_REALIGN_START, 1 | fdc.FDC_NO_AGGREGATE])) | (fdc.FDC_MAT_TILED if case % 2 else 0))
         ctx.fdc_destroy()
 
 
