@@ -400,6 +400,16 @@ def measure(b, args, peaks_cache, full):
                       "seconds_to_1pct_eq2": (sq_ms / nsq * 1e-3) * (mean_rel / 0.01) ** 2 if mean_rel > 0 else None,
                       "note": "PAPER.md:L116-118 context (GTX 295: +18 %, 1 % in about 2 minutes history-by-history); "
                               "seconds_to_1pct scales this run's time by (mean_rel / 1 %)^2"}
+        # eq. (2) as defined: the history's whole deposit in a voxel squared once (FDC_SQUARES_BY_HISTORY; per-thread table of
+        # visited voxels in local memory) -- same plan, same histories; the plain tally squares every stay (R10)
+        nh = min(3, args.steps) if base_ms < 100.0 else 1        # x 7 to x 24 the plain step: one timed step on the big configs
+        fh = b.flags | fdc.FDC_SQUARES_BY_HISTORY
+        b.timed(1, b.dose_d, flags=fh)
+        h_ms = b.timed(nh, b.dose_d, flags=fh)
+        flushes = ctx.fdc_last_call_info()["sq_history_flushes"]
+        mean_rel_h, n_avg_h = ctx.fdc_uncertainty_history(b.n_mine)
+        res["unc"].update({"ms_per_step_by_history": h_ms / nh, "squares_by_history_cost": h_ms / nh / base_ms - 1.0,
+                           "mean_rel_uncertainty_eq2_by_history": mean_rel_h, "by_history_table_flushes": flushes})
         ctx.fdc_reset()
 
     if b.rank == 0:
@@ -447,6 +457,9 @@ def per_config_entry(res, args):
          "reds_sent": roof["l2_atomic"]["reds_sent_per_step"], "clocks": res["clk"], "steps": args.steps, "warmup": max(args.warmup, 3)}
     if "unc" in res:
         e["squares_cost"] = res["unc"]["squares_cost"]; e["mean_rel_uncertainty_eq2"] = res["unc"]["mean_rel_uncertainty_eq2"]
+        e["squares_by_history_cost"] = res["unc"]["squares_by_history_cost"]
+        e["mean_rel_uncertainty_eq2_by_history"] = res["unc"]["mean_rel_uncertainty_eq2_by_history"]
+        e["by_history_table_flushes"] = res["unc"]["by_history_table_flushes"]
     return e
 
 

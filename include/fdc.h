@@ -114,6 +114,11 @@ enum {
                                   library's tiled copy of the material grid (4 x 4 x 1 voxels per 32-byte sector) ... */
     FDC_MAT_LINEAR     = 4096u,/* ... or from the x-fastest one.  Default: tiled iff the material and energy grids together
                                   (10 bytes per voxel) exceed the device's L2 cache */
+    FDC_SQUARES_BY_HISTORY = 8192u, /* implies FDC_TALLY_SQUARES; the squares tally follows eq. (2)'s definition: for
+                                  every history, everything it -- its primary and its secondaries -- left in a voxel is summed before
+                                  it is squared, whereas FDC_TALLY_SQUARES alone squares every uninterrupted stay in a voxel
+                                  (R10).  Each thread keeps the voxels its history has visited (up to 2048) in local
+                                  memory; slower */
     FDC_WARP_AGGREGATE = 1024u,/* scheduling only (same result): a small plan runs the latency-oriented instantiation that sums the
                                   shares of the lanes leaving the same voxel over the warp and sends one reduction per distinct
                                   voxel (north_star (4)), instead of the CTA-private tally; ignored for larger plans */
@@ -302,7 +307,8 @@ typedef struct {
     float ms_sort;           /* sampling-key + grouping kernels */
     float ms_gy;             /* Gy kernel (and the device-to-host copy of the dose grid, if any) */
     uint32_t launches;       /* kernels launched by the call */
-    uint32_t reserved;
+    uint32_t sq_history_flushes; /* FDC_SQUARES_BY_HISTORY runs since the last fdc_reset: histories whose table of visited voxels
+                                    filled up and was emptied early (such a history is squared in segments; 0 = eq. (2) exact) */
     uint64_t h2d_bytes;      /* bytes the call copied from host memory to the device (0 when the plan was cached) */
     uint64_t d2h_bytes;      /* bytes it copied back */
     uint64_t reds_sent;      /* FDC_DIAG_REDS runs since the last fdc_reset: 64-bit reductions actually sent */

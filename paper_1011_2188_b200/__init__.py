@@ -28,6 +28,7 @@ FDC_PRIVATE_TALLY = 512
 FDC_WARP_AGGREGATE = 1024
 FDC_MAT_TILED = 2048
 FDC_MAT_LINEAR = 4096
+FDC_SQUARES_BY_HISTORY = 8192
 
 FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH = 0, -1, -2, -3, -4, -5, -6
 
@@ -59,7 +60,7 @@ class _TrackDB(ctypes.Structure):
 
 class _CallInfo(ctypes.Structure):
     _fields_ = [("ms_total", ctypes.c_float), ("ms_transport", ctypes.c_float), ("ms_sort", ctypes.c_float), ("ms_gy", ctypes.c_float),
-                ("launches", ctypes.c_uint32), ("reserved", ctypes.c_uint32), ("h2d_bytes", ctypes.c_uint64), ("d2h_bytes", ctypes.c_uint64),
+                ("launches", ctypes.c_uint32), ("sq_history_flushes", ctypes.c_uint32), ("h2d_bytes", ctypes.c_uint64), ("d2h_bytes", ctypes.c_uint64),
                 ("reds_sent", ctypes.c_uint64), ("reds_traced", ctypes.c_uint64)]
 
 
@@ -317,7 +318,8 @@ class Fdc:
         ci = _CallInfo()
         self._check(self._lib.fdc_last_call_info(self._h, ctypes.byref(ci)))
         return {"total_ms": ci.ms_total, "transport_ms": ci.ms_transport, "sort_ms": ci.ms_sort, "gy_ms": ci.ms_gy, "launches": int(ci.launches),
-                "h2d_bytes": int(ci.h2d_bytes), "d2h_bytes": int(ci.d2h_bytes), "reds_sent": int(ci.reds_sent), "reds_traced": int(ci.reds_traced)}
+                "h2d_bytes": int(ci.h2d_bytes), "d2h_bytes": int(ci.d2h_bytes), "reds_sent": int(ci.reds_sent), "reds_traced": int(ci.reds_traced),
+                "sq_history_flushes": int(ci.sq_history_flushes)}
 
     def fdc_trace_reds(self, trace=None):
         """Diagnostics: a CUDA int32/uint32 tensor that FDC_DIAG_REDS runs fill with voxel indices (None removes it)."""

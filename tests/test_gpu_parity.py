@@ -297,6 +297,18 @@ def test_squares_bit_exact(fdc, which, request):
     with pytest.raises(fdc.FdcError) as e:
         ctx.fdc_run(w.beamlets, 0, 10, 1, w.seed, flags=1 | fdc.FDC_TALLY_SQUARES | fdc.FDC_NO_AGGREGATE)
     assert e.value.code == fdc.FDC_EINVAL
+    # eq. (2) as defined (FDC_SQUARES_BY_HISTORY): the history's whole deposit in a voxel squared once, equal to the oracle's
+    # by-history tally word for word, with the material read from either copy of the grid; the energy grid does not change
+    _, _, osh, _ = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, by_history=True)
+    for extra in (0, fdc.FDC_MAT_TILED, fdc.FDC_TALLY_SQUARES | fdc.FDC_NO_LAT):
+        ctx.fdc_reset()
+        ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed, flags=1 | fdc.FDC_SQUARES_BY_HISTORY | extra)
+        assert np.array_equal(ctx.fdc_get_sq_fixed(), osh) and np.array_equal(ctx.fdc_get_edep_fixed(), og)
+        assert ctx.fdc_last_call_info()["sq_history_flushes"] == 0
+        st_h = ctx.fdc_get_stats()
+        for k in STAT_KEYS:
+            assert st_h[k] == ost[k], (k, st_h[k], ost[k])
+    assert (osh >= osv).all()
     # additivity and reset
     g_a, s_a, _ = run_gpu_sq(fdc, ctx, w, first=0, n=w.n_protons // 3)
     ctx.fdc_run(w.beamlets, w.n_protons // 3, w.n_protons - w.n_protons // 3, 1, w.seed, flags=1 | fdc.FDC_TALLY_SQUARES)
@@ -304,6 +316,31 @@ def test_squares_bit_exact(fdc, which, request):
     ctx.fdc_reset()
     assert not ctx.fdc_get_sq_fixed().any()
     ctx.fdc_destroy()
+
+
+def test_squares_by_history_table_overflow(fdc):
+    """A history that visits more voxels than its table holds (2048): the table is emptied early and the event is counted.
+    Without re-entered voxels the tally still equals the definition; a track that comes back through the voxels of an earlier
+    segment is squared in segments -- between the per-stay and the per-history tallies, voxel by voxel."""
+    import oracle
+    from test_oracle_pins import hand_db, table_uniform
+    ph = fi.make_phantom("uniform", (2, 2, 6000), (1.0, 1.0, 1.0), hu0=0)
+    n = 64
+    for steps, exact in (([(0, 0, 5000.0, 5.0)], True), ([(0, 0, 5000.0, 5.0), (0, 0, -4999.0, 5.0)], False)):
+        w = fi.Workload("long", ph, table_uniform(1.0), hand_db([steps]), fi.single_beamlet((0.5, 0.5, 0.0), 100.0, 0.0, n), n, 9)
+        ctx = make_ctx(fdc, w)
+        ctx.fdc_run(w.beamlets, 0, n, 1, w.seed, flags=fdc.FDC_SQUARES_BY_HISTORY)
+        og, osv, osh, ost = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, flags=0, by_history=True)
+        s2 = ctx.fdc_get_sq_fixed()
+        assert np.array_equal(ctx.fdc_get_edep_fixed(), og)
+        assert ctx.fdc_last_call_info()["sq_history_flushes"] == n * (2 if exact else 4)
+        if exact:
+            assert np.array_equal(s2, osh) and np.array_equal(osh, osv)
+        else:
+            assert (s2 >= osv).all() and (s2 <= osh).all() and (s2 != osh).any() and (osh > osv).any()
+        ctx.fdc_reset()
+        assert ctx.fdc_last_call_info()["sq_history_flushes"] == 0
+        ctx.fdc_destroy()
 
 
 def test_uncertainty_history_and_batch(fdc):
@@ -608,8 +645,11 @@ def test_random_degenerate_worlds(fdc):
         if case % 4 == 0:
             ctx.fdc_reset()
             ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed, flags=1 | sq)
-            og, osv, _, _ = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, by_history=False)
+            og, osv, osh, _ = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, by_history=True)
             assert np.array_equal(ctx.fdc_get_edep_fixed(), og) and np.array_equal(ctx.fdc_get_sq_fixed(), osv), case
+            ctx.fdc_reset()                      # by history: these worlds have deflections beyond 90 degrees, i.e. re-entered voxels
+            ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed, flags=1 | fdc.FDC_SQUARES_BY_HISTORY | (fdc.FDC_MAT_TILED if case % 8 == 0 else 0))
+            assert np.array_equal(ctx.fdc_get_edep_fixed(), og) and np.array_equal(ctx.fdc_get_sq_fixed(), osh), case
         ctx.fdc_destroy()
 
 
@@ -627,8 +667,12 @@ def test_secondaries_bit_exact(fdc):
         ctx.fdc_reset()
         ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed, flags=flags)
         if flags & sq:
-            og, osv, _, ost = oracle.run_secondaries(w.phantom, w.table, db, sec, w.beamlets, w.seed, flags=flags & 33, squares=True)
+            og, osv, osh, ost = oracle.run_secondaries(w.phantom, w.table, db, sec, w.beamlets, w.seed, flags=flags & 33, squares=True)
             assert np.array_equal(ctx.fdc_get_sq_fixed(), osv)
+            # the same histories squared as eq. (2) defines them: parent and secondaries of a history summed per voxel first
+            ctx.fdc_reset()
+            ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed, flags=flags | fdc.FDC_SQUARES_BY_HISTORY)
+            assert np.array_equal(ctx.fdc_get_sq_fixed(), osh) and np.array_equal(ctx.fdc_get_edep_fixed(), og)
         else:
             og, ost = oracle.run_secondaries(w.phantom, w.table, db, sec, w.beamlets, w.seed, flags=flags & 33)
         st = ctx.fdc_get_stats()
@@ -687,5 +731,15 @@ def test_synthetic_secondaries_on_the_configs(fdc, wl2_small, wl3_small):
             assert st[k] == ost[k], (k, st[k], ost[k])
         g0, s0 = oracle.run(w0.phantom, w0.table, w0.db, w0.beamlets, w0.seed)
         assert ost["proton_steps"] > s0["proton_steps"] and ost["q_replayed"] > s0["q_replayed"]
+        # squares with secondaries: per stay (R10's reading) and per history (eq. (2) as defined) both equal the oracle's; here
+        # the two differ by percents of the tally (a parent and its secondary share the branch voxel), R10
+        _, osv, osh, _ = oracle.run_secondaries(w.phantom, w.table, db2, sec, w.beamlets, w.seed, squares=True)
+        ctx.fdc_reset(); ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed, flags=1 | fdc.FDC_TALLY_SQUARES)
+        assert np.array_equal(ctx.fdc_get_sq_fixed(), osv)
+        ctx.fdc_reset(); ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed, flags=1 | fdc.FDC_SQUARES_BY_HISTORY)
+        assert np.array_equal(ctx.fdc_get_sq_fixed(), osh) and np.array_equal(ctx.fdc_get_edep_fixed(), og)
+        assert ctx.fdc_last_call_info()["sq_history_flushes"] == 0
+        gap = 1.0 - float(osv.sum(dtype=np.float64)) / float(osh.sum(dtype=np.float64))
+        assert 0.005 < gap < 0.08, gap
         ctx.fdc_destroy()
 
