@@ -109,7 +109,8 @@ enum {
                                   that is emptied into the grid every few rounds (north_star (4)); meant to be
                                   used with FDC_SORT_SPATIAL; ignored with FDC_TALLY_SQUARES / FDC_NO_AGGREGATE */
     FDC_NO_LAT         = 256u, /* debug: run a small plan (at most one wave of thread blocks) through the same instantiation as a
-                                  large one; by default it runs with the CTA-private tally of FDC_PRIVATE_TALLY (same result) */
+                                  large one; by default it runs with the CTA-private tally of FDC_PRIVATE_TALLY in blocks sized at launch so
+                                  that its warps spread evenly over the SMs (same result) */
     FDC_MAT_TILED      = 2048u,/* scheduling only (same result): the transport kernel reads the material of the voxel ahead from the
                                   library's tiled copy of the material grid (4 x 4 x 1 voxels per 32-byte sector) ... */
     FDC_MAT_LINEAR     = 4096u,/* ... or from the x-fastest one.  Default: tiled iff the material and energy grids together
