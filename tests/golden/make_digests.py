@@ -6,7 +6,7 @@ same plan through the CUDA path on the box and compares digests.  Calls only ora
 input generators (fdc_inputs); proton ranges are spread over threads (integer sums: any split gives
 the same grid, pin P7).
 
-    python tests/golden/make_digests.py [3 4 5]
+    python tests/golden/make_digests.py [3 4 5]      (sq3: only the squares digests of config 3)
 """
 import hashlib
 import json
@@ -55,30 +55,41 @@ def digest(cfg, threads):
 
 
 def digest_squares(cfg, threads):
-    """The sum-of-squares grid (R10, by visit) of the whole plan: sha256 of its u64 bytes and its sum."""
+    """The sum-of-squares grids (R10) of the whole plan, per stay and per history (eq. (2) as defined): sha256 of the u64 bytes
+    and the sums."""
     w = fi.workload(cfg, lazy_db=True)
     parts = threads * 4
     bounds = [w.n_protons * k // parts for k in range(parts + 1)]
 
     def work(k):
-        g, sq, _, st = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, first=bounds[k], n=bounds[k + 1] - bounds[k], by_history=False)
-        return sq
+        g, sq, sqh, st = oracle.run_sq(w.phantom, w.table, w.db, w.beamlets, w.seed, first=bounds[k], n=bounds[k + 1] - bounds[k], by_history=True)
+        return sq, sqh
 
     total = np.zeros(w.phantom.hu.shape, dtype=np.uint64)
+    total_h = np.zeros(w.phantom.hu.shape, dtype=np.uint64)
     with ThreadPoolExecutor(threads) as ex:
-        for sq in ex.map(work, range(parts)):
+        for sq, sqh in ex.map(work, range(parts)):
             total += sq
+            total_h += sqh
+    assert (total_h >= total).all()
     return {"sha256_u64_squares": hashlib.sha256(np.ascontiguousarray(total).tobytes()).hexdigest(),
-            "squares_sum_mod_2_64": int(total.sum(dtype=np.uint64))}
+            "squares_sum_mod_2_64": int(total.sum(dtype=np.uint64)),
+            "sha256_u64_squares_by_history": hashlib.sha256(np.ascontiguousarray(total_h).tobytes()).hexdigest(),
+            "squares_by_history_sum_mod_2_64": int(total_h.sum(dtype=np.uint64))}
 
 
 if __name__ == "__main__":
-    cfgs = [int(a) for a in sys.argv[1:]] or [3, 4, 5]
+    args = sys.argv[1:] or ["3", "4", "5"]
     data = json.load(open(OUT)) if os.path.exists(OUT) else {}
-    for c in cfgs:
-        data[str(c)] = digest(c, threads=os.cpu_count() or 1)
-        if c == 3:                                   # the squares tally at full size on the one-field plan
+    for a in args:
+        if a.startswith("sq"):                       # "sq3": only the squares digests of a config whose plain digest is stored
+            c = int(a[2:])
             data[str(c)].update(digest_squares(c, threads=os.cpu_count() or 1))
+        else:
+            c = int(a)
+            data[str(c)] = digest(c, threads=os.cpu_count() or 1)
+            if c == 3:                               # the squares tallies at full size on the one-field plan
+                data[str(c)].update(digest_squares(c, threads=os.cpu_count() or 1))
         print(c, data[str(c)]["sha256_u64_grid"], data[str(c)]["oracle_seconds"], "s", flush=True)
         with open(OUT, "w") as f:
             json.dump(data, f, indent=1, sort_keys=True)

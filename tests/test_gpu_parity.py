@@ -538,6 +538,14 @@ def test_full_plan_digest(fdc, cfg):
         assert int(sq.sum(dtype=np.uint64)) == d["squares_sum_mod_2_64"]
         assert hashlib.sha256(np.ascontiguousarray(sq).tobytes()).hexdigest() == d["sha256_u64_squares"]
         assert np.array_equal(ctx.fdc_get_edep_fixed(), g)
+    if "sha256_u64_squares_by_history" in d:           # eq. (2) as defined, at full size
+        ctx.fdc_reset()
+        ctx.fdc_run(w.beamlets, 0, w.n_protons, 1, w.seed, flags=1 | fdc.FDC_SQUARES_BY_HISTORY)
+        assert ctx.fdc_last_call_info()["sq_history_flushes"] == 0
+        sq = ctx.fdc_get_sq_fixed()
+        assert int(sq.sum(dtype=np.uint64)) == d["squares_by_history_sum_mod_2_64"]
+        assert hashlib.sha256(np.ascontiguousarray(sq).tobytes()).hexdigest() == d["sha256_u64_squares_by_history"]
+        assert np.array_equal(ctx.fdc_get_edep_fixed(), g)
     ctx.fdc_destroy()
 
 
