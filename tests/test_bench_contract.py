@@ -32,3 +32,19 @@ def test_product_arm_refuses_to_run_without_a_gpu():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1", "--warmup", "0"],
                          capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert out.returncode != 0 and "no CPU fallback" in (out.stderr + out.stdout)
+
+
+def test_static_ncu_counts_point_at_committed_captures():
+    """roofline.traffic / roofline.ncu come from profiles/r02_counts.csv: one row per config, each naming a summary that is
+    committed under profiles/ and the commit of the kernel it was captured from (which the summary's header repeats)."""
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.HEADLINE_CONFIG == 5
+    for cfg in (1, 2, 3, 4, 5):
+        sc = bench._static_counts(cfg)
+        assert sc is not None, cfg
+        assert sc["dram_bytes"] > 0 and sc["warp_instructions"] > 0 and sc["kernel_ms_under_ncu"] > 0
+        path = os.path.join(ROOT, sc["source"])
+        assert os.path.exists(path), path
+        head = open(path).read(4000)
+        assert sc["kernel_commit"] in head and "ncu --set full" in head and "k_transport<" in head
