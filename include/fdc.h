@@ -113,8 +113,9 @@ enum {
                                   that its warps spread evenly over the SMs (same result) */
     FDC_MAT_TILED      = 2048u,/* scheduling only (same result): the transport kernel reads the material of the voxel ahead from the
                                   library's tiled copy of the material grid (4 x 4 x 1 voxels per 32-byte sector) ... */
-    FDC_MAT_LINEAR     = 4096u,/* ... or from the x-fastest one.  Default: tiled iff the material and energy grids together
-                                  (10 bytes per voxel) exceed the device's L2 cache */
+    FDC_MAT_LINEAR     = 4096u,/* ... or from the x-fastest one.  Default, per launch: tiled for an oblique field (second direction
+                                  component >= 0.3), or if the material and energy grids together (10 bytes per voxel) exceed the
+                                  device's L2 cache */
     FDC_SQUARES_BY_HISTORY = 8192u, /* implies FDC_TALLY_SQUARES; the squares tally follows eq. (2)'s definition: for
                                   every history, everything it -- its primary and its secondaries -- left in a voxel is summed before
                                   it is squared, whereas FDC_TALLY_SQUARES alone squares every uninterrupted stay in a voxel
