@@ -264,7 +264,9 @@ class Bench:
         t_track = st["proton_steps"] * STEP_RECORD_BYTES / (hbm_gbs * 1e9)
         t_atomic = st["deposits"] / (ceilings["peak_gred_s"] * 1e9)
         bound_atomic = t_atomic >= t_track
-        n_chunks = max(1, -(-self.n_mine // (1 << 25)))
+        # transport launches per step: the library cuts a run at 2^25 protons and at field boundaries; each launch comes with 5
+        # sort kernels, and the step ends with one Gy kernel
+        n_chunks = max(1, (int(infos[-1]["launches"]) - 1) // 6) if self.world == 1 else max(1, int(infos[-1]["launches"]) // 6)
         la = dict(ceilings)
         la.update({"achieved_gred_s": st["deposits"] / (tr_ms * 1e-3) / 1e9,
                    "sent_gred_s": ceilings["reds_sent_per_step"] / (tr_ms * 1e-3) / 1e9,
