@@ -295,6 +295,44 @@ int fdc_profile(fdc_ctx *ctx, const float *values, int axis, int fixed_a, int fi
 int fdc_rms_diff(fdc_ctx *ctx, const float *dose_ref, const float *dose_eval, double *rms_over_max, double *max_ref);
 
 /* ------------------------------------------------------------------------------------------------------------
+ * Eq. (1) without any device allocation.
+ *
+ * Who this is for.  The paper's way of using the batch estimate is a loop: run a batch, evaluate eq. (1), stop
+ * once the mean dose uncertainty is below the target.  A planning service that runs this
+ * loop in steady state has often given every byte of device memory to its own arena at start-up (or lives inside
+ * a host framework whose caching allocator has), so a cudaMalloc made on its behalf either fails or takes memory
+ * the arena believes it owns; and cudaFree waits for all work on the device (cudaMalloc may too), which a loop
+ * that overlaps the next batch's transport with this evaluation cannot afford.  fdc_uncertainty_batch
+ * allocates its scratch lazily (a pointer table, four accumulator words, and a whole float grid when rel_sigma is a
+ * host array), so such callers cannot know when it will allocate.  This call never does: it makes no cudaMalloc,
+ * cudaFree or allocating library call, on any path.
+ *
+ * How.  Its scratch is a fixed FDC_NOALLOC_SCRATCH_BYTES (512) array that is part of the library image: every GPU
+ * on which libfdc.so gets loaded holds those bytes until the process exits, whether or not this call is used.
+ * Words 0-2 are the reduction accumulators (maximum dose, fixed-point sum, voxel count), the second half is the
+ * table of batch-grid pointers.  Hence the limit: 2 <= n_batches <= FDC_NOALLOC_MAX_BATCHES (32; the paper uses
+ * 6); more is refused with FDC_EINVAL and a message naming the limit (fdc_uncertainty_batch takes up to 64).
+ *
+ * Arguments and results are those of fdc_uncertainty_batch (same kernel, same arithmetic, bit-identical
+ * *mean_rel, *n_voxels_averaged and rel_sigma), except that rel_sigma_dev is a DEVICE array of nx*ny*nz floats
+ * or NULL: the caller owns every input and output, the library only borrows them for the call.  batch_grids is
+ * a HOST array of DEVICE pointers.  Synchronises the context's stream before it returns.
+ *
+ * First call on a device.  The address of the array on the context's device is looked up once per device, by the
+ * first call made with a context on that device (cudaGetSymbolAddress, with that device current); that call may
+ * initialise the CUDA module, so make it once during set-up, before any stream capture is begun.
+ *
+ * Sharing.  There is ONE array per device, shared by every context and every call in the process.  A call
+ * clears the accumulators it needs and overwrites the pointers it uses; it keeps nothing from call to call.
+ * Two calls whose device work overlaps in time (different contexts / streams / host threads on one device)
+ * race on it and both results are garbage: serialise them.  Calls on different devices do not interact.
+ * ------------------------------------------------------------------------------------------------------------ */
+#define FDC_NOALLOC_MAX_BATCHES 32
+#define FDC_NOALLOC_SCRATCH_BYTES 512
+int fdc_uncertainty_batch_noalloc(fdc_ctx *ctx, const uint64_t *const *batch_grids, int n_batches, uint64_t histories_per_batch,
+                                  float *rel_sigma_dev, double *mean_rel, uint64_t *n_voxels_averaged);
+
+/* ------------------------------------------------------------------------------------------------------------
  * Diagnostics.  NOT part of the method and not among the calls SURVEY §8(b) lists: they report what the library
  * did, for bench.py's timing split, its end-to-end byte counts and its contention-limited roofline ceiling.  The
  * roofline microbenchmarks themselves live in a separate library (csrc/bench_peaks.cu -> libfdcpeaks.so).

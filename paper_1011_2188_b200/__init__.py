@@ -30,12 +30,14 @@ FDC_MAT_TILED = 2048
 FDC_MAT_LINEAR = 4096
 FDC_SQUARES_BY_HISTORY = 8192
 
+FDC_NOALLOC_MAX_BATCHES = 32          # fdc_uncertainty_batch_noalloc: what its fixed scratch holds
+
 FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = ["fdc_create", "fdc_load_tracks", "fdc_run", "fdc_to_gy", "fdc_get_edep_fixed", "fdc_set_edep_fixed", "fdc_edep_device_ptr",
            "fdc_get_stats", "fdc_reset", "fdc_destroy", "fdc_strerror", "fdc_last_error",
            "fdc_get_sq_fixed", "fdc_set_sq_fixed", "fdc_uncertainty_history", "fdc_uncertainty_batch", "fdc_run_phase_space", "fdc_gamma_index",
-           "fdc_profile", "fdc_rms_diff", "fdc_set_secondaries",
+           "fdc_profile", "fdc_rms_diff", "fdc_set_secondaries", "fdc_uncertainty_batch_noalloc",
            "fdc_last_call_info", "fdc_trace_reds"]          # the last two: diagnostics (include/fdc.h)
 
 BEAMLET_DTYPE = np.dtype([("origin", "<f4", 3), ("e1", "<f4", 3), ("e2", "<f4", 3), ("dir", "<f4", 3),
@@ -126,6 +128,8 @@ def lib():
         L.fdc_uncertainty_history.argtypes = [vp, u64, vp, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
         L.fdc_uncertainty_batch.restype = i32
         L.fdc_uncertainty_batch.argtypes = [vp, vp, i32, u64, vp, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
+        L.fdc_uncertainty_batch_noalloc.restype = i32
+        L.fdc_uncertainty_batch_noalloc.argtypes = [vp, vp, i32, u64, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64)]
         _lib = L
     return _lib
 
@@ -294,6 +298,20 @@ class Fdc:
         self._check(self._lib.fdc_uncertainty_batch(self._h, ctypes.cast(ptrs, ctypes.c_void_p), len(batch_grids), int(histories_per_batch),
                                                     _ptr(rel_sigma), 1 if (rel_sigma is not None and _is_device(rel_sigma)) else 0,
                                                     ctypes.byref(m), ctypes.byref(c)))
+        return m.value, int(c.value)
+
+    def fdc_uncertainty_batch_noalloc(self, batch_grids, histories_per_batch, rel_sigma=None):
+        """Eq. (1) for callers that must not cause a device allocation while they run (all device memory handed to
+        their own arena, or no room for the device-wide wait a cudaMalloc / cudaFree can bring): same results as
+        fdc_uncertainty_batch, scratch in a fixed 512-byte array inside the library, at most FDC_NOALLOC_MAX_BATCHES
+        grids.  rel_sigma: None or a CUDA float32 tensor [nz,ny,nx] the caller owns.  One scratch array per device:
+        calls that overlap on the GPU race.  Make the first call on a device during set-up (include/fdc.h)."""
+        assert all(_is_device(g) and g.is_contiguous() for g in batch_grids)
+        assert rel_sigma is None or (_is_device(rel_sigma) and rel_sigma.is_contiguous())
+        ptrs = (ctypes.c_void_p * len(batch_grids))(*[g.data_ptr() for g in batch_grids])
+        m = ctypes.c_double(0.0); c = ctypes.c_uint64(0)
+        self._check(self._lib.fdc_uncertainty_batch_noalloc(self._h, ctypes.cast(ptrs, ctypes.c_void_p), len(batch_grids),
+                                                            int(histories_per_batch), _ptr(rel_sigma), ctypes.byref(m), ctypes.byref(c)))
         return m.value, int(c.value)
 
     def fdc_gamma_index(self, dose_ref, dose_eval, dose_tol_frac=0.03, dist_tol_mm=3.0, search_mm=None, cutoff_frac=0.0, gamma_out=None):
