@@ -45,6 +45,8 @@ def sharded_step(ctx, beamlets, first, n_mine, seed, flags, dose_out, world):
         ctx.fdc_run(beamlets, first, n_mine, 1, seed, flags=flags, dose_gy=dose_out)
         return
     ctx.fdc_run(beamlets, first, n_mine, 1, seed, flags=flags)
-    allreduce_edep(ctx, squares=bool(flags & 16))          # 16 = FDC_TALLY_SQUARES
+    # FDC_SQUARES_BY_HISTORY alone also fills the squares grid (the library implies FDC_TALLY_SQUARES)
+    from . import FDC_SQUARES_BY_HISTORY, FDC_TALLY_SQUARES
+    allreduce_edep(ctx, squares=bool(flags & (FDC_TALLY_SQUARES | FDC_SQUARES_BY_HISTORY)))
     if dose_out is not None:
         ctx.fdc_to_gy(dose_out)

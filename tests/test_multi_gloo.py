@@ -80,8 +80,10 @@ class _OracleCtx:
     def fdc_run(self, beamlets, first, n, stride, seed, flags=1, dose_gy=None):
         import oracle
         w = self.w
-        if flags & 16:
-            g, sq, _, _ = oracle.run_sq(w.phantom, w.table, w.db, beamlets, seed, first=first, n=n, stride=stride, flags=flags & 33, by_history=False)
+        if flags & (16 | 8192):                 # FDC_SQUARES_BY_HISTORY (8192) implies the squares grid, as in the library
+            g, sq, sqh, _ = oracle.run_sq(w.phantom, w.table, w.db, beamlets, seed, first=first, n=n, stride=stride, flags=flags & 33,
+                                          by_history=bool(flags & 8192))
+            sq = sqh if flags & 8192 else sq
             if self.sq is None:
                 self.sq = np.zeros(w.phantom.hu.shape, dtype=np.uint64)
             self.sq += sq
@@ -116,6 +118,8 @@ def _step_worker(rank, world, store, out_dir):
     assert ctx.calls == ["reset", "run", "gy"] * 2
     np.save(os.path.join(out_dir, "dose%d.npy" % rank), dose)
     np.save(os.path.join(out_dir, "sq%d.npy" % rank), ctx.sq)
+    sharded_step(ctx, w.beamlets, first, n, w.seed, 1 | 8192, dose, world)      # the by-history flag alone
+    np.save(os.path.join(out_dir, "sqh%d.npy" % rank), ctx.sq)
     dist.barrier()
     dist.destroy_process_group()
 
@@ -131,6 +135,7 @@ def test_sharded_step_control_flow_world_2():
         mp.spawn(_step_worker, args=(2, os.path.join(d, "store"), d), nprocs=2, join=True)
         doses = [np.load(os.path.join(d, "dose%d.npy" % r)) for r in range(2)]
         sqs = [np.load(os.path.join(d, "sq%d.npy" % r)) for r in range(2)]
+        sqhs = [np.load(os.path.join(d, "sqh%d.npy" % r)) for r in range(2)]
     w = fi.workload(3, n_protons=1176, tracks_per_bin=20)
     one = _OracleCtx(w)
     dose1 = np.zeros(w.phantom.hu.shape, dtype=np.float32)
@@ -138,6 +143,9 @@ def test_sharded_step_control_flow_world_2():
     assert one.calls == ["reset", "run", "gy"]
     assert dose1.any() and np.array_equal(doses[0], dose1) and np.array_equal(doses[1], dose1)
     assert np.array_equal(sqs[0], one.sq) and np.array_equal(sqs[1], one.sq)
+    # FDC_SQUARES_BY_HISTORY without FDC_TALLY_SQUARES: the squares grid is summed over ranks all the same
+    sharded_step(one, w.beamlets, 0, w.n_protons, w.seed, 1 | 8192, dose1, 1)
+    assert one.sq.any() and np.array_equal(sqhs[0], one.sq) and np.array_equal(sqhs[1], one.sq)
 
 
 def test_bench_refuses_a_world_size_that_contradicts_gpus():
