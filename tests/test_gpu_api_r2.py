@@ -120,7 +120,7 @@ def test_call_info_counts_the_copies(fdc, wl3_small):
     w = wl3_small
     ctx = make_ctx(fdc, w)
     nb = len(w.beamlets)
-    plan_bytes = nb * (72 + 20) + (nb + 1) * 8          # beamlets + their sort-key records + prefix sums
+    plan_bytes = nb * 72 + (nb + 1) * 8                 # beamlets + prefix sums
     ctx.fdc_run(w.beamlets, 0, 100, 1, w.seed)
     a = ctx.fdc_last_call_info()
     assert a["h2d_bytes"] == plan_bytes and a["d2h_bytes"] == 0 and a["launches"] == 6 and a["transport_ms"] > 0
@@ -130,7 +130,39 @@ def test_call_info_counts_the_copies(fdc, wl3_small):
     dose = np.zeros(w.phantom.hu.shape, dtype=np.float32)
     ctx.fdc_run(bl2, 200, 100, 1, w.seed, dose_gy=dose)
     c = ctx.fdc_last_call_info()
-    assert c["h2d_bytes"] == plan_bytes + 100 and c["d2h_bytes"] == dose.nbytes and c["launches"] == 7
+    assert c["h2d_bytes"] == plan_bytes + 80 and c["d2h_bytes"] == dose.nbytes and c["launches"] == 7
+    # the per-beamlet sort-key records (20 B) exist only for plans run with FDC_SORT_SPATIAL: uploaded by the first such run
+    ctx.fdc_run(bl2, 300, 100, 1, w.seed, flags=1 | fdc.FDC_SORT_SPATIAL)
+    assert ctx.fdc_last_call_info()["h2d_bytes"] == (nb + 1) * 20
+    ctx.fdc_run(bl2, 400, 100, 1, w.seed, flags=1 | fdc.FDC_SORT_SPATIAL)
+    assert ctx.fdc_last_call_info()["h2d_bytes"] == 0
+    ctx.fdc_destroy()
+
+
+@pytest.mark.timeout(180)
+@pytest.mark.parametrize("n_bl", [3000, 300_000])
+def test_spatial_sort_with_one_group_per_beamlet(fdc, wl3_small, n_bl):
+    """a plan in which every beamlet has its own origin is its own sort group.  3 000 groups fit the key
+    space (3 000 x 256 keys); 300 000 do not (> 2^24 keys: the library groups by track instead) and used to cost
+    n^2/2 comparisons on the host.  FDC_SORT_SPATIAL is scheduling only: the grid equals the plain run's bit for bit."""
+    w = wl3_small
+    src = w.beamlets[len(w.beamlets) // 2]
+    bl = np.repeat(src[None], n_bl).copy()
+    step = np.float32(1e-4) * np.arange(n_bl, dtype=np.float32)                 # distinct origins along e1, 30 mm at most
+    bl["origin"] = src["origin"][None, :] + step[:, None] * src["e1"][None, :]
+    assert len(np.unique(bl["origin"], axis=0)) == n_bl
+    bl["n_protons"] = 1
+    ctx = make_ctx(fdc, w)
+    ctx.fdc_run(bl, 0, n_bl, 1, w.seed, flags=1)
+    plain, st_plain = ctx.fdc_get_edep_fixed(), ctx.fdc_get_stats()
+    ctx.fdc_reset()
+    ctx.fdc_run(bl[:-1], 0, n_bl - 1, 1, w.seed, flags=1)                        # another plan in between: the cache forgets
+    ctx.fdc_reset()
+    ctx.fdc_run(bl, 0, n_bl, 1, w.seed, flags=1 | fdc.FDC_SORT_SPATIAL)
+    info = ctx.fdc_last_call_info()
+    assert info["h2d_bytes"] == n_bl * 72 + (n_bl + 1) * 8 + (n_bl * 20 if n_bl == 3000 else 0)
+    assert np.array_equal(ctx.fdc_get_edep_fixed(), plain) and ctx.fdc_get_stats() == st_plain
+    assert st_plain["protons"] == n_bl and st_plain["deposits"] > 0
     ctx.fdc_destroy()
 
 
