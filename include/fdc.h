@@ -92,7 +92,11 @@ enum {
     FDC_ERANGE    = -3,   /* beamlet energy above the top bin, or its bin is empty */
     FDC_ENOMEM    = -4,
     FDC_ECUDA     = -5,   /* CUDA error; text via fdc_last_error */
-    FDC_EARCH     = -6    /* device is not compute capability 10.x (no fallback by design) */
+    FDC_EARCH     = -6,   /* device is not compute capability 10.x (no fallback by design) */
+    /* positive codes are warnings: the call did its work and every output is valid; fdc_last_error says what to know */
+    FDC_WSEGMENTED = 1    /* fdc_uncertainty_history: the squares grid holds FDC_SQUARES_BY_HISTORY runs in which some histories
+                             visited more voxels than the per-history table holds and were squared in segments, so for them
+                             eq. (2)'s D_i^2 is a sum of squares of partial sums (between the per-stay and the exact tally) */
 };
 
 enum {
@@ -233,7 +237,8 @@ int fdc_set_sq_fixed(fdc_ctx *ctx, const uint64_t *grid_in, int is_device_ptr);
  * rel_sigma (may be NULL): nx*ny*nz floats, host or device per rel_is_device_ptr.  *mean_rel: the
  * paper's "mean dose uncertainty" (L92): the average of rel over the voxels whose dose m/rho
  * exceeds half the maximum dose; *n_voxels_averaged: how many.  Synchronises.  FDC_EINVAL if
- * n_histories < 2 or no squares grid exists.
+ * n_histories < 2 or no squares grid exists.  Returns FDC_WSEGMENTED (> 0, outputs valid) instead of FDC_OK when
+ * FDC_SQUARES_BY_HISTORY runs since the last fdc_reset emptied a history's table early (fdc_call_info.sq_history_flushes > 0).
  */
 int fdc_uncertainty_history(fdc_ctx *ctx, uint64_t n_histories, float *rel_sigma, int rel_is_device_ptr,
                             double *mean_rel, uint64_t *n_voxels_averaged);

@@ -33,6 +33,7 @@ FDC_SQUARES_BY_HISTORY = 8192
 FDC_NOALLOC_MAX_BATCHES = 32          # fdc_uncertainty_batch_noalloc: what its fixed scratch holds
 
 FDC_OK, FDC_EINVAL, FDC_ENOTRACKS, FDC_ERANGE, FDC_ENOMEM, FDC_ECUDA, FDC_EARCH = 0, -1, -2, -3, -4, -5, -6
+FDC_WSEGMENTED = 1                    # positive codes are warnings: outputs valid (include/fdc.h)
 
 EXPORTS = ["fdc_create", "fdc_load_tracks", "fdc_run", "fdc_to_gy", "fdc_get_edep_fixed", "fdc_set_edep_fixed", "fdc_edep_device_ptr",
            "fdc_get_stats", "fdc_reset", "fdc_destroy", "fdc_strerror", "fdc_last_error",
@@ -51,6 +52,10 @@ class FdcError(RuntimeError):
     def __init__(self, code, msg):
         super().__init__("fdc error %d: %s" % (code, msg))
         self.code = code
+
+
+class FdcWarning(RuntimeWarning):
+    """A positive return code of the library: the call did its work, its outputs are valid."""
 
 
 class _TrackDB(ctypes.Structure):
@@ -185,6 +190,10 @@ class Fdc:
         self._h = h
 
     def _check(self, rc):
+        if rc > 0:
+            import warnings
+            warnings.warn(FdcWarning("fdc warning %d: %s: %s" % (rc, self._lib.fdc_strerror(rc).decode(), self._lib.fdc_last_error(self._h).decode())), stacklevel=3)
+            return
         if rc != 0:
             raise FdcError(rc, "%s: %s" % (self._lib.fdc_strerror(rc).decode(), self._lib.fdc_last_error(self._h).decode()))
 

@@ -334,12 +334,20 @@ def test_squares_by_history_table_overflow(fdc):
         s2 = ctx.fdc_get_sq_fixed()
         assert np.array_equal(ctx.fdc_get_edep_fixed(), og)
         assert ctx.fdc_last_call_info()["sq_history_flushes"] == n * (2 if exact else 4)
+        with pytest.warns(fdc.FdcWarning, match="squared in segments"):          # the overflow is not silent (FDC_WSEGMENTED)
+            mean_w, cnt_w = ctx.fdc_uncertainty_history(n)
+        assert cnt_w > 0 and mean_w >= 0.0                                        # outputs valid all the same
         if exact:
             assert np.array_equal(s2, osh) and np.array_equal(osh, osv)
         else:
             assert (s2 >= osv).all() and (s2 <= osh).all() and (s2 != osh).any() and (osh > osv).any()
         ctx.fdc_reset()
         assert ctx.fdc_last_call_info()["sq_history_flushes"] == 0
+        ctx.fdc_run(w.beamlets, 0, n, 1, w.seed, flags=fdc.FDC_TALLY_SQUARES)     # per stay: no table, no warning
+        import warnings
+        with warnings.catch_warnings():
+            warnings.simplefilter("error")
+            ctx.fdc_uncertainty_history(n)
         ctx.fdc_destroy()
 
 
