@@ -36,5 +36,21 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+CHECKED_LIB = os.path.join(HERE, "libfdc_checked.so")
+
+
+def build_checked() -> str:
+    """libfdc_checked.so: the same source with -DFDC_CHECKED (device-side asserts on every material, step-record and tally
+    address; csrc/fdc.cu).  Not built by default; run the GPU tests on it with FDC_LIB=<this path>."""
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    tmp = CHECKED_LIB + ".tmp.%d" % os.getpid()
+    subprocess.check_call([nvcc] + NVCC_FLAGS + ["-DFDC_CHECKED", "-o", tmp, SRC])
+    os.replace(tmp, CHECKED_LIB)
+    return CHECKED_LIB
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--checked" in sys.argv:
+        print(build_checked())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
