@@ -54,19 +54,34 @@ def _peaks():
 
 
 def _static_counts(cfg):
-    """ncu figures that cannot be measured live (DRAM bytes, warp instructions of one launch): the newest capture
-    of this config's transport kernel, written by hand from profiles/ into profiles/r02_counts.csv with the commit
-    of the kernel it was taken from."""
-    p = os.path.join(ROOT, "profiles", "r02_counts.csv")
+    """ncu figures that cannot be measured live: profiles/r03_counts.csv holds one row per k_transport launch of one timed
+    step of every config (ncu --metrics, profiles/r03_README.md), with the commit of the kernel.  Returned: the step's sums
+    (DRAM bytes, warp instructions, kernel time under ncu) and the TIME-WEIGHTED means over its launches of the L2 tag-request
+    rate and the issue-active share (VERDICT r2 #6: not one launch of six)."""
+    p = os.path.join(ROOT, "profiles", "r03_counts.csv")
     if not os.path.exists(p):
         return None
     with open(p) as f:
-        rows = [l.split(",") for l in f.read().splitlines()[1:] if l.strip() and not l.startswith("#")]
-    for c in rows:
-        if c[0].strip() == str(cfg):
-            return {"launch": c[1].strip(), "dram_bytes": float(c[2]), "warp_instructions": float(c[3]), "kernel_ms_under_ncu": float(c[4]),
-                    "source": c[5].strip(), "kernel_commit": c[6].strip()}
-    return None
+        lines = [l for l in f.read().splitlines() if l.strip() and not l.startswith("#")]
+    hdr = lines[0].split(",")
+    rows = [dict(zip(hdr, l.split(","))) for l in lines[1:]]
+    rows = [r for r in rows if r["config"].strip() == str(cfg)]
+    if not rows:
+        return None
+    ms = [float(r["kernel_ms_under_ncu"]) for r in rows]
+    tot = sum(ms)
+    wmean = lambda k: sum(float(r[k]) * t for r, t in zip(rows, ms)) / tot      # noqa: E731
+    dram = sum(float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]) for r in rows)
+    return {"launch": "all %d k_transport launches of one timed step" % len(rows), "n_launches": len(rows),
+            "dram_bytes": dram / len(rows), "dram_bytes_per_step": dram,
+            "warp_instructions": sum(float(r["warp_instructions"]) for r in rows) / len(rows),
+            "warp_instructions_per_step": sum(float(r["warp_instructions"]) for r in rows),
+            "kernel_ms_under_ncu": tot / len(rows), "kernel_ms_per_step_under_ncu": tot,
+            "l2_tag_pct_time_weighted": wmean("l2_tag_requests_avg_pct"), "l2_tag_pct_hottest_slice_time_weighted": wmean("l2_tag_requests_max_pct"),
+            "issue_active_pct_time_weighted": wmean("issue_active_pct"), "warps_active_pct_time_weighted": wmean("warps_active_pct"),
+            "l2_red_requests_per_step": sum(float(r["l2_red_requests"]) for r in rows),
+            "l2_red_lookup_miss_share": sum(float(r["l2_red_sectors_lookup_miss"]) for r in rows) / sum(float(r["l2_red_sectors"]) for r in rows),
+            "per_launch_ms": ms, "source": "profiles/r03_counts.csv", "kernel_commit": rows[0]["kernel_commit"].strip()}
 
 
 class ClockSampler:
@@ -337,12 +352,20 @@ class Bench:
             mhz = (clk or {}).get("sm_mhz") or 1965.0
             peak_issue = 148 * 4 * mhz * 1e6
             roof["traffic"] = sc["dram_bytes"]
-            roof["ncu"] = {"launch": sc["launch"], "dram_bytes_per_launch": sc["dram_bytes"], "warp_instructions_per_launch": sc["warp_instructions"],
-                           "kernel_ms_under_ncu": sc["kernel_ms_under_ncu"],
-                           "issue_frac_under_ncu": sc["warp_instructions"] / (sc["kernel_ms_under_ncu"] * 1e-3) / (148 * 4 * 1965e6),
+            roof["ncu"] = {"launch": sc["launch"], "dram_bytes_per_launch": sc["dram_bytes"], "dram_bytes_per_step": sc["dram_bytes_per_step"],
+                           "warp_instructions_per_launch": sc["warp_instructions"], "warp_instructions_per_step": sc["warp_instructions_per_step"],
+                           "kernel_ms_under_ncu": sc["kernel_ms_under_ncu"], "kernel_ms_per_step_under_ncu": sc["kernel_ms_per_step_under_ncu"],
+                           "per_launch_ms_under_ncu": sc["per_launch_ms"],
+                           "issue_frac_under_ncu": sc["warp_instructions_per_step"] / (sc["kernel_ms_per_step_under_ncu"] * 1e-3) / (148 * 4 * 1965e6),
+                           "issue_active_pct_time_weighted": sc["issue_active_pct_time_weighted"],
+                           "warps_active_pct_time_weighted": sc["warps_active_pct_time_weighted"],
+                           "l2_tag_pct_time_weighted": sc["l2_tag_pct_time_weighted"],
+                           "l2_tag_pct_hottest_slice_time_weighted": sc["l2_tag_pct_hottest_slice_time_weighted"],
+                           "l2_red_requests_per_step": sc["l2_red_requests_per_step"], "l2_red_lookup_miss_share": sc["l2_red_lookup_miss_share"],
                            "source": sc["source"], "kernel_commit": sc["kernel_commit"],
-                           "note": "static: one ncu --set full capture of ONE launch of this config (profiles/), not measured in this run; "
-                                   "issue_frac = warp instructions / (time x 148 SMs x 4 schedulers x 1965 MHz)"}
+                           "note": "static: ncu --metrics capture of EVERY k_transport launch of one timed step of this config (profiles/), not "
+                                   "measured in this run; per-launch figures are the step's sums / launches, percentages are weighted by launch "
+                                   "time; issue_frac = warp instructions / (time x 148 SMs x 4 schedulers x 1965 MHz)"}
             roof["issue_peak_ginst_s_at_sampled_clock"] = peak_issue / 1e9
         return roof
 

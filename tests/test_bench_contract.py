@@ -1,6 +1,7 @@
 """bench.py's reference arm runs without a GPU: one JSON line with the keys the driver reads."""
 import json
 import os
+import re
 import subprocess
 import sys
 
@@ -35,16 +36,18 @@ def test_product_arm_refuses_to_run_without_a_gpu():
 
 
 def test_static_ncu_counts_point_at_committed_captures():
-    """roofline.traffic / roofline.ncu come from profiles/r02_counts.csv: one row per config, each naming a summary that is
-    committed under profiles/ and the commit of the kernel it was captured from (which the summary's header repeats)."""
+    """roofline.traffic / roofline.ncu come from profiles/r03_counts.csv: one row per k_transport launch of one timed step of
+    every config (1 / 1 / 1 / 3 / 6 launches), with the commit of the kernel; the README beside it names the ncu command."""
     sys.path.insert(0, ROOT)
     import bench
     assert bench.HEADLINE_CONFIG == 5
-    for cfg in (1, 2, 3, 4, 5):
+    for cfg, n in ((1, 1), (2, 1), (3, 1), (4, 3), (5, 6)):
         sc = bench._static_counts(cfg)
         assert sc is not None, cfg
+        assert sc["n_launches"] == n and len(sc["per_launch_ms"]) == n
         assert sc["dram_bytes"] > 0 and sc["warp_instructions"] > 0 and sc["kernel_ms_under_ncu"] > 0
-        path = os.path.join(ROOT, sc["source"])
-        assert os.path.exists(path), path
-        head = open(path).read(4000)
-        assert sc["kernel_commit"] in head and "ncu --set full" in head and "k_transport<" in head
+        assert 0 < sc["l2_tag_pct_time_weighted"] <= sc["l2_tag_pct_hottest_slice_time_weighted"] <= 100
+        assert os.path.exists(os.path.join(ROOT, sc["source"]))
+        assert re.fullmatch(r"[0-9a-f]{7,12}", sc["kernel_commit"])
+    readme = open(os.path.join(ROOT, "profiles", "r03_README.md")).read()
+    assert "r03_counts.csv" in readme and "ncu --clock-control none -k regex:k_transport" in readme and "bench.py --config" in readme
